@@ -1,0 +1,466 @@
+/*
+ * gray2_oracle.c -- CPU ORACLE for the GRay2 hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, double precision.  Shares nothing with the CUDA path.  See gray2_oracle.h.
+ * Every function cites the passage of /root/reference/PAPER.md (arXiv:1706.07062) it follows;
+ * "DESIGN Rn" refers to the numbered readings in DESIGN.md where the paper is silent.
+ *
+ * Parity pins (tests/test_oracle_*.py): eq.(5) residual, l.l=1, g g^-1 = 1, Schwarzschild limit,
+ * central differences of the metric, Gamma symmetry, Newtonian limit, conservation rates,
+ * Table 1 of the paper, 4th-order convergence, photon sphere,
+ * circular-orbit period, ISCO, epicyclic frequency, Bardeen shadow, Carter radial potential,
+ * independent Boyer-Lindquist integration.  No function is "parity unpinned".
+ */
+#include "gray2_oracle.h"
+#include <math.h>
+#include <stddef.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ------------------------------------------------------------------------------------------
+ * C1.  Kerr-Schild radius r(x,y,z), eq. (5):
+ *        x^2 + y^2 + z^2 = r^2 + a^2 (1 - z^2/r^2)
+ *      multiplied by r^2:  r^4 - (R^2 - a^2) r^2 - a^2 z^2 = 0,  positive root for r^2.
+ * ---------------------------------------------------------------------------------------- */
+double oracle_ks_r(double a, double x, double y, double z)
+{
+  double R2 = x * x + y * y + z * z;
+  double w = R2 - a * a;
+  double r2 = 0.5 * (w + sqrt(w * w + 4.0 * a * a * z * z));
+  return sqrt(r2);
+}
+
+/* f and l_alpha of PAPER.md:59-61, eq. (3)-(4) (M = 1). */
+static void ks_f_l(double a, const double pos[3], double *r_out, double *f_out, double l[4])
+{
+  double x = pos[0], y = pos[1], z = pos[2];
+  double r = oracle_ks_r(a, x, y, z);
+  double r2 = r * r;
+  *r_out = r;
+  *f_out = 2.0 * r2 * r / (r2 * r2 + a * a * z * z);
+  l[0] = 1.0;
+  l[1] = (r * x + a * y) / (r2 + a * a);
+  l[2] = (r * y - a * x) / (r2 + a * a);
+  l[3] = z / r;
+}
+
+static const double ETA[4] = { -1.0, 1.0, 1.0, 1.0 };
+
+/* PAPER.md:55 eq. (2): g_ab = eta_ab + f l_a l_b. */
+void oracle_ks_metric(double a, const double pos[3], double g[16])
+{
+  double r, f, l[4];
+  ks_f_l(a, pos, &r, &f, l);
+  for (int i = 0; i < 4; ++i)
+    for (int j = 0; j < 4; ++j)
+      g[i * 4 + j] = (i == j ? ETA[i] : 0.0) + f * l[i] * l[j];
+}
+
+/* Inverse of a Kerr-Schild metric: g^ab = eta^ab - f l^a l^b, l^a = eta^ab l_b (l is null).
+ * Not printed in the paper; pinned in tests by g * g^-1 = 1. */
+void oracle_ks_metric_inverse(double a, const double pos[3], double gi[16])
+{
+  double r, f, l[4], lu[4];
+  ks_f_l(a, pos, &r, &f, l);
+  for (int i = 0; i < 4; ++i) lu[i] = ETA[i] * l[i];
+  for (int i = 0; i < 4; ++i)
+    for (int j = 0; j < 4; ++j)
+      gi[i * 4 + j] = (i == j ? ETA[i] : 0.0) - f * lu[i] * lu[j];
+}
+
+/* C2.  Analytic first derivatives of the metric, d_c g_ab, by implicit differentiation of eq. (5):
+ *   d_i r = f x_i / 2 (i = x,y),  d_z r = f z (r^2+a^2) / (2 r^2)
+ *   d_i f = f [ (3/r - 2 f) d_i r - delta_iz 2 a^2 z / (r^4 + a^2 z^2) ]
+ *   d_j l_x = [ d_j r (x - 2 r l_x) + r delta_jx + a delta_jy ] / (r^2+a^2)
+ *   d_j l_y = [ d_j r (y - 2 r l_y) + r delta_jy - a delta_jx ] / (r^2+a^2)
+ *   d_j l_z = ( delta_jz - l_z d_j r ) / r ,  d_j l_0 = 0 ,  d_t (anything) = 0.
+ * Then d_c g_ab = (d_c f) l_a l_b + f (d_c l_a) l_b + f l_a (d_c l_b)   (64 numbers).
+ * Layout: dg[c*16 + a*4 + b], c = derivative index (0 = t). */
+void oracle_ks_dmetric(double a, const double pos[3], double dg[64])
+{
+  double x = pos[0], y = pos[1], z = pos[2];
+  double r, f, l[4];
+  ks_f_l(a, pos, &r, &f, l);
+  double r2 = r * r, P = r2 + a * a, S = r2 * r2 + a * a * z * z;
+  double dr[4], df[4], dl[4][4]; /* dr[c], df[c], dl[c][alpha] ; index 0 = t */
+  dr[0] = 0.0;
+  dr[1] = 0.5 * f * x;
+  dr[2] = 0.5 * f * y;
+  dr[3] = 0.5 * f * z * P / r2;
+  for (int c = 0; c < 4; ++c) {
+    double dcz = (c == 3) ? 1.0 : 0.0, dcx = (c == 1) ? 1.0 : 0.0, dcy = (c == 2) ? 1.0 : 0.0;
+    df[c] = f * ((3.0 / r - 2.0 * f) * dr[c] - dcz * 2.0 * a * a * z / S);
+    dl[c][0] = 0.0;
+    dl[c][1] = (dr[c] * (x - 2.0 * r * l[1]) + r * dcx + a * dcy) / P;
+    dl[c][2] = (dr[c] * (y - 2.0 * r * l[2]) + r * dcy - a * dcx) / P;
+    dl[c][3] = (dcz - l[3] * dr[c]) / r;
+  }
+  df[0] = 0.0;
+  for (int al = 0; al < 4; ++al) dl[0][al] = 0.0;
+  for (int c = 0; c < 4; ++c)
+    for (int i = 0; i < 4; ++i)
+      for (int j = 0; j < 4; ++j)
+        dg[c * 16 + i * 4 + j] = df[c] * l[i] * l[j] + f * dl[c][i] * l[j] + f * l[i] * dl[c][j];
+}
+
+/* Plainer variant: central differences of the metric itself (no analytic derivative at all). */
+void oracle_ks_dmetric_fd(double a, const double pos[3], double step, double dg[64])
+{
+  double gp[16], gm[16], p[3];
+  for (int k = 0; k < 16; ++k) dg[k] = 0.0; /* d_t g = 0 : metric is stationary */
+  for (int c = 1; c < 4; ++c) {
+    memcpy(p, pos, sizeof p);
+    p[c - 1] = pos[c - 1] + step; oracle_ks_metric(a, p, gp);
+    p[c - 1] = pos[c - 1] - step; oracle_ks_metric(a, p, gm);
+    for (int k = 0; k < 16; ++k) dg[c * 16 + k] = (gp[k] - gm[k]) / (2.0 * step);
+  }
+}
+
+/* PAPER.md:91 eq. (8): Gamma^m_ab = 1/2 g^{m nu} ( g_{nu a,b} + g_{nu b,a} - g_{ab,nu} ). */
+static void christoffel_from(const double gi[16], const double dg[64], double Gam[64])
+{
+  for (int m = 0; m < 4; ++m)
+    for (int al = 0; al < 4; ++al)
+      for (int be = 0; be < 4; ++be) {
+        double s = 0.0;
+        for (int nu = 0; nu < 4; ++nu)
+          s += gi[m * 4 + nu] * (dg[be * 16 + nu * 4 + al] + dg[al * 16 + nu * 4 + be] - dg[nu * 16 + al * 4 + be]);
+        Gam[m * 16 + al * 4 + be] = 0.5 * s;
+      }
+}
+
+void oracle_ks_christoffel(double a, const double pos[3], double Gam[64])
+{
+  double gi[16], dg[64];
+  oracle_ks_metric_inverse(a, pos, gi);
+  oracle_ks_dmetric(a, pos, dg);
+  christoffel_from(gi, dg, Gam);
+}
+
+/* PAPER.md:87 eq. (7): xdd^m = - Gamma^m_ab xd^a xd^b, full triple loop, no regrouping. */
+static void accel_from(const double Gam[64], const double u[4], double acc[4])
+{
+  for (int m = 0; m < 4; ++m) {
+    double s = 0.0;
+    for (int al = 0; al < 4; ++al)
+      for (int be = 0; be < 4; ++be)
+        s += Gam[m * 16 + al * 4 + be] * u[al] * u[be];
+    acc[m] = -s;
+  }
+}
+
+void oracle_ks_accel(double a, const double pos[3], const double u[4], double acc[4])
+{
+  double Gam[64];
+  oracle_ks_christoffel(a, pos, Gam);
+  accel_from(Gam, u, acc);
+}
+
+void oracle_ks_accel_fd(double a, const double pos[3], const double u[4], double step, double acc[4])
+{
+  double gi[16], dg[64], Gam[64];
+  oracle_ks_metric_inverse(a, pos, gi);
+  oracle_ks_dmetric_fd(a, pos, step, dg);
+  christoffel_from(gi, dg, Gam);
+  accel_from(Gam, u, acc);
+}
+
+/* C4.  y = (t,x,y,z,u^t,u^x,u^y,u^z);  y' = (u^mu, xdd^mu(x^i,u^mu)).  Autonomous. */
+static void ks_deriv(double a, const double y[8], double dy[8])
+{
+  for (int m = 0; m < 4; ++m) dy[m] = y[4 + m];
+  oracle_ks_accel(a, &y[1], &y[4], &dy[4]);
+}
+
+/* "classic 4th-order Runge-Kutta".
+ *   k1 = y'(y), k2 = y'(y + h/2 k1), k3 = y'(y + h/2 k2), k4 = y'(y + h k3),
+ *   y <- y + h/6 (k1 + 2 k2 + 2 k3 + k4). */
+typedef void (*deriv_fn)(double a, const double y[8], double dy[8]);
+
+static void rk4_generic(deriv_fn F, double a, double y[8], double h)
+{
+  double k1[8], k2[8], k3[8], k4[8], w[8];
+  F(a, y, k1);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + 0.5 * h * k1[i];
+  F(a, w, k2);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + 0.5 * h * k2[i];
+  F(a, w, k3);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + h * k3[i];
+  F(a, w, k4);
+  for (int i = 0; i < 8; ++i) y[i] = y[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+}
+
+void oracle_rk4_step(double a, double y[8], double h) { rk4_generic(ks_deriv, a, y, h); }
+
+void oracle_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out)
+{
+  double y[8];
+  memcpy(y, y0, sizeof y);
+  memcpy(out, y, sizeof y);
+  int64_t rec = 1;
+  for (int64_t s = 1; s <= nsteps; ++s) {
+    oracle_rk4_step(a, y, h);
+    if (s % stride == 0) { memcpy(out + 8 * rec, y, sizeof y); ++rec; }
+  }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C7.  Invariants.  u_0 = -u^0 + f U,  u_i = u^i + f l_i U,  U = l_a u^a  (index lowered with eq. 2).
+ *   norm = u_a u^a                       (the paper's error indicator u^2)
+ *   E    = -u_0                          (d_t is Killing)
+ *   L_z  = x u_y - y u_x                 (x d_y - y d_x is Killing: rotating phi_KS rotates x+iy)
+ *   Q    = u_theta^2 + cos^2(theta) [ a^2 (mu^2 - E^2) + L_z^2 / sin^2(theta) ]   (Carter; Table 1 "Q")
+ * written without 1/sin(theta) (DESIGN R8), c = z/r, s^2 = 1 - c^2, P = r^2 + a^2:
+ *   Q = P c^2 (u_x^2+u_y^2) - 2 r c (x u_x + y u_y) u_z + r^2 s^2 u_z^2 + a^2 c^2 (mu^2 - E^2)
+ * mu^2 is the NOMINAL value from `kind` (0 null, 1 time-like).
+ * ---------------------------------------------------------------------------------------- */
+void oracle_invariants_one(double a, int32_t kind, const double y[8], double out[4])
+{
+  double r, f, l[4], g[16], ulow[4];
+  const double *u = &y[4];
+  ks_f_l(a, &y[1], &r, &f, l);
+  oracle_ks_metric(a, &y[1], g);
+  for (int i = 0; i < 4; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < 4; ++j) s += g[i * 4 + j] * u[j];
+    ulow[i] = s;
+  }
+  double norm = 0.0;
+  for (int i = 0; i < 4; ++i) norm += ulow[i] * u[i];
+  double E = -ulow[0];
+  double x = y[1], yy = y[2], z = y[3];
+  double Lz = x * ulow[2] - yy * ulow[1];
+  double c = z / r, s2 = 1.0 - c * c, P = r * r + a * a;
+  double mu2 = (kind == ORACLE_TIMELIKE) ? 1.0 : 0.0;
+  double Q = P * c * c * (ulow[1] * ulow[1] + ulow[2] * ulow[2])
+           - 2.0 * r * c * (x * ulow[1] + yy * ulow[2]) * ulow[3]
+           + r * r * s2 * ulow[3] * ulow[3]
+           + a * a * c * c * (mu2 - E * E);
+  out[0] = E; out[1] = Lz; out[2] = Q; out[3] = norm;
+}
+
+int oracle_invariants(const oracle_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm)
+{
+  if (!s || n == 0 || n > s->n || !E || !Lz || !Q || !norm) return 1;
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < (int64_t)n; ++k) {
+    double y[8], o[4];
+    for (int m = 0; m < 8; ++m) y[m] = s->q[m][k];
+    oracle_invariants_one(s->a_eff, s->kind, y, o);
+    E[k] = o[0]; Lz[k] = o[1]; Q[k] = o[2]; norm[k] = o[3];
+  }
+  return 0;
+}
+
+/* u^t from g_ab u^a u^b = -mu^2 given the spatial components (future-directed root), DESIGN R3:
+ *   -(u^t)^2 + |u|^2 + f (u^t + c)^2 = -mu^2 ,  c = l_i u^i
+ *   (1-f) (u^t)^2 - 2 f c u^t - (|u|^2 + mu^2 + f c^2) = 0
+ *   u^t = [ f c + sqrt( f^2 c^2 + (1-f)(|u|^2 + mu^2 + f c^2) ) ] / (1-f)      (needs f < 1) */
+static double solve_ut(double a, const double pos[3], const double v[3], double mu2)
+{
+  double r, f, l[4];
+  ks_f_l(a, pos, &r, &f, l);
+  double c = l[1] * v[0] + l[2] * v[1] + l[3] * v[2];
+  double A = 1.0 - f, B = f * c, C = v[0] * v[0] + v[1] * v[1] + v[2] * v[2] + mu2 + f * c * c;
+  return (B + sqrt(B * B + A * C)) / A;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Image-plane initial conditions ("integrate backwards null geodesics from an image
+ * at an initial radius"; the construction itself is not in the paper: DESIGN R1-R3).
+ *  R1 pixel centres: alpha_j = -Wa + (j+1/2) 2Wa/nx ; beta_k likewise ; index = k*nx + j.
+ *  R2 observer direction n = (sin i, 0, cos i), e_alpha = (0,1,0), e_beta = (-cos i, 0, sin i);
+ *     position = r_obs n + alpha e_alpha + beta e_beta in Cartesian KS ; t = 0 ; parallel rays.
+ *  R3 the backward trace is run as the time-reversed forward problem: spin a_eff = -a,
+ *     spatial tangent -n (unit Euclidean length), u^t = future-directed null root, dir = +1.
+ * ---------------------------------------------------------------------------------------- */
+int oracle_init_null(oracle_state *s, double a, double r_obs, double inc,
+                     double Wa, double Wb, int32_t nx, int32_t ny)
+{
+  if (!s || nx <= 0 || ny <= 0 || (uint64_t)nx * (uint64_t)ny != s->n) return 1;
+  if (!(fabs(a) <= 1.0) || !(r_obs > 1.0 + sqrt(1.0 - a * a))) return 1;
+  double ae = -a;
+  s->a_eff = ae; s->kind = ORACLE_NULL; s->reversed = 1;
+  double si = sin(inc), ci = cos(inc);
+  double nvec[3] = { si, 0.0, ci }, ea[3] = { 0.0, 1.0, 0.0 }, eb[3] = { -ci, 0.0, si };
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < ny; ++k)
+    for (int64_t j = 0; j < nx; ++j) {
+      double alpha = -Wa + ((double)j + 0.5) * (2.0 * Wa / (double)nx);
+      double beta  = -Wb + ((double)k + 0.5) * (2.0 * Wb / (double)ny);
+      double pos[3], v[3];
+      for (int c = 0; c < 3; ++c) {
+        pos[c] = r_obs * nvec[c] + alpha * ea[c] + beta * eb[c];
+        v[c] = -nvec[c];
+      }
+      int64_t idx = k * nx + j;
+      s->q[0][idx] = 0.0;
+      s->q[1][idx] = pos[0]; s->q[2][idx] = pos[1]; s->q[3][idx] = pos[2];
+      s->q[4][idx] = solve_ut(ae, pos, v, 0.0);
+      s->q[5][idx] = v[0]; s->q[6][idx] = v[1]; s->q[7][idx] = v[2];
+      s->lambda[idx] = 0.0; s->status[idx] = ORACLE_ACTIVE; s->nsteps[idx] = 0;
+    }
+  return 0;
+}
+
+/* Explicit 8-vectors ("8 variables"; PAPER.md:263 explicit v_z kick).  xu8 is AoS n x 8.
+ * renormalise_ut != 0 re-solves u^t from g u u = -1 (DESIGN R7). */
+int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renorm)
+{
+  if (!s || !xu8 || n == 0 || n > s->n || !(fabs(a) <= 1.0)) return 1;
+  s->a_eff = a; s->kind = ORACLE_TIMELIKE; s->reversed = 0;
+  for (uint64_t k = 0; k < n; ++k) {
+    for (int m = 0; m < 8; ++m) s->q[m][k] = xu8[k * 8 + m];
+    if (renorm) s->q[4][k] = solve_ut(a, &xu8[k * 8 + 1], &xu8[k * 8 + 5], 1.0);
+    s->lambda[k] = 0.0; s->status[k] = ORACLE_ACTIVE; s->nsteps[k] = 0;
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C5.  Driver loop for one geodesic (stopping rule PAPER.md:296-302: "pass by or are close enough
+ * to the event horizon, or escape"; step rule and order of tests: DESIGN R4-R6).
+ * ---------------------------------------------------------------------------------------- */
+static int all_finite(const double y[8])
+{
+  for (int i = 0; i < 8; ++i) if (!isfinite(y[i])) return 0;
+  return 1;
+}
+
+static void integrate_one(double a, double y[8], double *lambda, int32_t *status, int32_t *nsteps,
+                          double lambda_end, const oracle_step_control *sc)
+{
+  double r_plus = 1.0 + sqrt(1.0 - a * a);
+  double dir = (double)sc->dir;
+  while (*status == ORACLE_ACTIVE) {
+    double r = oracle_ks_r(a, y[1], y[2], y[3]);
+    if (!isfinite(r) || !all_finite(y)) { *status = ORACLE_INVALID; break; }
+    if (r < sc->capture_factor * r_plus) { *status = ORACLE_CAPTURED; break; }
+    if (r > sc->r_escape)                { *status = ORACLE_ESCAPED;  break; }
+    if (*nsteps >= sc->max_steps)        { *status = ORACLE_MAXSTEPS; break; }
+    if (dir * (lambda_end - *lambda) <= 0.0) break; /* stays ACTIVE: resumable */
+    double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
+    if (fabs(h) > fabs(lambda_end - *lambda)) h = lambda_end - *lambda; /* clip the last step */
+    oracle_rk4_step(a, y, h);
+    *lambda += h;
+    *nsteps += 1;
+  }
+}
+
+int oracle_integrate(oracle_state *s, uint64_t n, double lambda_end,
+                     const oracle_step_control *sc, oracle_stats *stats)
+{
+  if (!s || !sc || n == 0 || n > s->n) return 1;
+  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return 1;
+  if (sc->dir != 1 && sc->dir != -1) return 1;
+  uint64_t steps = 0, nc = 0, ne = 0, nm = 0, ni = 0, na = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : steps, nc, ne, nm, ni, na)
+  for (int64_t k = 0; k < (int64_t)n; ++k) {
+    double y[8];
+    for (int m = 0; m < 8; ++m) y[m] = s->q[m][k];
+    int32_t st = s->status[k], ns = s->nsteps[k], ns0 = ns;
+    double lam = s->lambda[k];
+    integrate_one(s->a_eff, y, &lam, &st, &ns, lambda_end, sc);
+    for (int m = 0; m < 8; ++m) s->q[m][k] = y[m];
+    s->status[k] = st; s->nsteps[k] = ns; s->lambda[k] = lam;
+    steps += (uint64_t)(ns - ns0);
+    nc += (st == ORACLE_CAPTURED); ne += (st == ORACLE_ESCAPED); nm += (st == ORACLE_MAXSTEPS);
+    ni += (st == ORACLE_INVALID);  na += (st == ORACLE_ACTIVE);
+  }
+  if (stats) {
+    stats->steps = steps; stats->n_captured = nc; stats->n_escaped = ne;
+    stats->n_maxsteps = nm; stats->n_invalid = ni; stats->n_active = na;
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C8.  Independent Boyer-Lindquist integrator (oracle self-check only).
+ * PAPER.md:47 eq. (1), M = 1, coordinates X = (t, r, theta, phi):
+ *   ds^2 = -(1 - 2r/rho^2) dt^2 - (4 r a sin^2/rho^2) dphi dt + (rho^2/Delta) dr^2 + rho^2 dtheta^2
+ *          + (r^2 + a^2 + 2 r a^2 sin^2/rho^2) sin^2 dphi^2 ,
+ *   rho^2 = r^2 + a^2 cos^2(theta),  Delta = r^2 - 2 r + a^2.
+ * Metric derivatives by 4th-order central differences, inverse by Gauss-Jordan, then the same
+ * eq. (8) and eq. (7) routines as above.  Nothing Kerr-Schild specific is used.
+ * ---------------------------------------------------------------------------------------- */
+void oracle_bl_metric(double a, const double X[4], double g[16])
+{
+  double r = X[1], th = X[2];
+  double st = sin(th), ct = cos(th), s2 = st * st;
+  double rho2 = r * r + a * a * ct * ct, Delta = r * r - 2.0 * r + a * a;
+  for (int k = 0; k < 16; ++k) g[k] = 0.0;
+  g[0 * 4 + 0] = -(1.0 - 2.0 * r / rho2);
+  g[0 * 4 + 3] = g[3 * 4 + 0] = -2.0 * r * a * s2 / rho2;
+  g[1 * 4 + 1] = rho2 / Delta;
+  g[2 * 4 + 2] = rho2;
+  g[3 * 4 + 3] = (r * r + a * a + 2.0 * r * a * a * s2 / rho2) * s2;
+}
+
+static void invert4(const double m[16], double inv[16])
+{
+  double A[4][8];
+  for (int i = 0; i < 4; ++i)
+    for (int j = 0; j < 4; ++j) { A[i][j] = m[i * 4 + j]; A[i][4 + j] = (i == j) ? 1.0 : 0.0; }
+  for (int c = 0; c < 4; ++c) {
+    int p = c;
+    for (int i = c + 1; i < 4; ++i) if (fabs(A[i][c]) > fabs(A[p][c])) p = i;
+    if (p != c) for (int j = 0; j < 8; ++j) { double t = A[c][j]; A[c][j] = A[p][j]; A[p][j] = t; }
+    double d = A[c][c];
+    for (int j = 0; j < 8; ++j) A[c][j] /= d;
+    for (int i = 0; i < 4; ++i) if (i != c) {
+      double fct = A[i][c];
+      for (int j = 0; j < 8; ++j) A[i][j] -= fct * A[c][j];
+    }
+  }
+  for (int i = 0; i < 4; ++i) for (int j = 0; j < 4; ++j) inv[i * 4 + j] = A[i][4 + j];
+}
+
+void oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4])
+{
+  double g[16], gi[16], dg[64], Gam[64];
+  oracle_bl_metric(a, X, g);
+  invert4(g, gi);
+  for (int k = 0; k < 64; ++k) dg[k] = 0.0;
+  for (int c = 1; c <= 2; ++c) { /* metric depends on r and theta only */
+    double step = 1e-3 * (c == 1 ? fmax(1.0, fabs(X[1])) : 1.0);
+    double Y[4], g1p[16], g1m[16], g2p[16], g2m[16];
+    memcpy(Y, X, sizeof Y);
+    Y[c] = X[c] + step;       oracle_bl_metric(a, Y, g1p);
+    Y[c] = X[c] - step;       oracle_bl_metric(a, Y, g1m);
+    Y[c] = X[c] + 2.0 * step; oracle_bl_metric(a, Y, g2p);
+    Y[c] = X[c] - 2.0 * step; oracle_bl_metric(a, Y, g2m);
+    for (int k = 0; k < 16; ++k)
+      dg[c * 16 + k] = (8.0 * (g1p[k] - g1m[k]) - (g2p[k] - g2m[k])) / (12.0 * step);
+  }
+  christoffel_from(gi, dg, Gam);
+  accel_from(Gam, u, acc);
+}
+
+static void bl_deriv(double a, const double y[8], double dy[8])
+{
+  for (int m = 0; m < 4; ++m) dy[m] = y[4 + m];
+  oracle_bl_accel(a, &y[0], &y[4], &dy[4]);
+}
+
+void oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out)
+{
+  double y[8];
+  memcpy(y, y0, sizeof y);
+  memcpy(out, y, sizeof y);
+  int64_t rec = 1;
+  for (int64_t s = 1; s <= nsteps; ++s) {
+    rk4_generic(bl_deriv, a, y, h);
+    if (s % stride == 0) { memcpy(out + 8 * rec, y, sizeof y); ++rec; }
+  }
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}

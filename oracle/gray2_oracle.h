@@ -1,0 +1,86 @@
+/*
+ * gray2_oracle.h -- CPU ORACLE for the GRay2 hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * This library is the slow, plain, double-precision statement of what the CUDA path
+ * (include/gray2.h) must compute.  It shares no code with the CUDA path and is never
+ * called by it.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.
+ *
+ * It follows the paper (arXiv:1706.07062, /root/reference/PAPER.md) literally:
+ *   metric      g = eta + f l l               PAPER.md:55-66  (eq. 2-5)
+ *   derivatives analytic d_c g_ab             implicit differentiation of eq. (5)
+ *   connection  Gamma = 1/2 g^-1 (dg+dg-dg)   PAPER.md:91     (eq. 8)
+ *   geodesic    xdd = -Gamma xd xd            PAPER.md:87     (eq. 7), full 4x4x4 loop
+ *   stepper     classic 4th-order Runge-Kutta PAPER.md:164
+ * It does NOT use the regrouped eq. (10)-(14) form; that is the CUDA side's formula.
+ *
+ * Units G = c = M = 1.  All arrays are HOST memory owned by the caller.
+ * Parity pins: see DESIGN.md "Oracle pins"; no function here is "parity unpinned".
+ */
+#ifndef GRAY2_ORACLE_H
+#define GRAY2_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORACLE_ACTIVE = 0, ORACLE_CAPTURED = 1, ORACLE_ESCAPED = 2, ORACLE_MAXSTEPS = 3, ORACLE_INVALID = 4 };
+enum { ORACLE_NULL = 0, ORACLE_TIMELIKE = 1 };
+
+typedef struct {
+  double  *q[8];      /* t,x,y,z,u^t,u^x,u^y,u^z : n doubles each (SoA)             */
+  double  *lambda;    /* n : affine parameter reached                               */
+  int32_t *status;    /* n : ORACLE_ACTIVE ...                                      */
+  int32_t *nsteps;    /* n : RK4 steps taken so far                                 */
+  uint64_t n;
+  double   a_eff;     /* spin used by the integrator (= -a for reversed rays)       */
+  int32_t  kind;      /* ORACLE_NULL / ORACLE_TIMELIKE (nominal mu^2 for Carter Q)  */
+  int32_t  reversed;  /* 1: time-reversed ray of a backward trace                   */
+} oracle_state;
+
+typedef struct {
+  int32_t mode;            /* 0: h = dir*h_fixed ; 1: h = dir*eta*r (KS r at step start) */
+  double  h_fixed, eta;
+  int32_t dir;             /* +1 or -1                                                   */
+  double  capture_factor;  /* CAPTURED when r < capture_factor * r_plus                  */
+  double  r_escape;        /* ESCAPED  when r > r_escape (+inf allowed)                  */
+  int32_t max_steps;       /* per-ray total                                              */
+} oracle_step_control;
+
+typedef struct { uint64_t steps, n_captured, n_escaped, n_maxsteps, n_invalid, n_active; } oracle_stats;
+
+/* ---- the four operations of the boundary, on host arrays ---- */
+int oracle_init_null(oracle_state *s, double a, double r_obs, double inclination_rad,
+                     double fov_half_alpha, double fov_half_beta, int32_t nx, int32_t ny);
+int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renormalise_ut);
+int oracle_integrate(oracle_state *s, uint64_t n, double lambda_end,
+                     const oracle_step_control *sc, oracle_stats *stats /* may be NULL */);
+int oracle_invariants(const oracle_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm);
+
+/* ---- building blocks, exported so that the tests can pin each of them ---- */
+double oracle_ks_r(double a, double x, double y, double z);                         /* eq. (5)            */
+void   oracle_ks_metric(double a, const double pos[3], double g[16]);               /* eq. (2)-(4)        */
+void   oracle_ks_metric_inverse(double a, const double pos[3], double gi[16]);      /* eta - f l^a l^b    */
+void   oracle_ks_dmetric(double a, const double pos[3], double dg[64]);             /* dg[c*16+a*4+b]     */
+void   oracle_ks_dmetric_fd(double a, const double pos[3], double step, double dg[64]); /* central diffs  */
+void   oracle_ks_christoffel(double a, const double pos[3], double Gam[64]);        /* Gam[m*16+a*4+b]    */
+void   oracle_ks_accel(double a, const double pos[3], const double u[4], double acc[4]);        /* eq. (7) */
+void   oracle_ks_accel_fd(double a, const double pos[3], const double u[4], double step, double acc[4]);
+void   oracle_rk4_step(double a, double y[8], double h);                            /* one RK4 step       */
+void   oracle_invariants_one(double a, int32_t kind, const double y[8], double out[4]); /* E,Lz,Q,norm   */
+/* fixed-step trajectory: writes y after every `stride` steps (and the initial state first):
+   out has (nsteps/stride + 1) * 8 doubles. */
+void   oracle_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out);
+
+/* ---- independent Boyer-Lindquist integrator (self-check only; eq. 1) ---- */
+void   oracle_bl_metric(double a, const double X[4], double g[16]);                 /* X = t,r,theta,phi  */
+void   oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4]);
+void   oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out);
+
+int    oracle_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
