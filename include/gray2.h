@@ -1,0 +1,133 @@
+/*
+ * gray2.h -- C-ABI of the B200-native batched Kerr-Schild geodesic integrator
+ *            (data-parallel hot path of GRay2, Chan et al. 2017, arXiv:1706.07062).
+ *
+ * "PAPER.md:N" cites line N of the paper text; "DESIGN Rn" the numbered readings in DESIGN.md that
+ * fill the points the paper leaves open.  Units G = c = M = 1.
+ *
+ * What is computed (all of it in CUDA kernels for sm_100a; there is no CPU fallback):
+ *   gray2_init_null      image-plane initial conditions of null geodesics      PAPER.md:296; DESIGN R1-R3
+ *   gray2_init_timelike  explicit 8-vectors (t,x,y,z,u^t,u^x,u^y,u^z)
+ *   gray2_integrate      classic RK4 of the geodesic equation in Cartesian Kerr-Schild
+ *                        coordinates, metric g = eta + f l l (eq. 2-5), right-hand side in
+ *                        the regrouped form of eq. (10)-(14), each geodesic advanced
+ *                        until it is close to the horizon, escapes, or exhausts its step budget
+ *
+ *   gray2_invariants     E, L_z, Carter Q and u.u ("u^2"; Table 1 "Phi", "Q")
+ *
+ * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
+ * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
+ * library allocates no persistent memory of its own except one 64-byte work-queue scratch per process,
+ * and temporary staging inside gray2_init_timelike (freed stream-ordered).  `host_xu8` is a HOST pointer.
+ * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
+ *
+ * Asynchrony.  Every call enqueues on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
+ * stream) and returns; results are valid after the caller synchronises that stream.
+ *
+ * Errors.  Every call returns a gray2_err; nothing throws or aborts.  GRAY2_EINVAL: bad argument
+ * (NULL pointer, n == 0, |a| > 1, r_obs <= r_plus, nx*ny != s->n, eta <= 0, prec mismatch, ...).
+ * GRAY2_ESTATE: n larger than s->n.  GRAY2_ECUDA: a CUDA runtime error (text via gray2_last_error()).
+ * Numerical trouble of a single geodesic is data (status GRAY2_INVALID), never an error.
+ *
+ * Determinism.  No arithmetic crosses geodesics: every output element depends only on that geodesic's
+ * input, not on scheduling, so results are bit-reproducible run to run.
+ */
+#ifndef GRAY2_H
+#define GRAY2_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { GRAY2_F64 = 0, GRAY2_F32 = 1 } gray2_precision;
+typedef enum { GRAY2_NULL = 0, GRAY2_TIMELIKE = 1 } gray2_kind;        /* nominal mu^2 = 0 or 1 */
+typedef enum { GRAY2_ACTIVE = 0, GRAY2_CAPTURED = 1, GRAY2_ESCAPED = 2,
+               GRAY2_MAXSTEPS = 3, GRAY2_INVALID = 4 } gray2_ray_status;
+typedef enum { GRAY2_OK = 0, GRAY2_EINVAL = 1, GRAY2_ESTATE = 2, GRAY2_ECUDA = 3 } gray2_err;
+
+/* State of n geodesics, structure of arrays (8 variables per geodesic; SoA: PAPER.md:316). */
+typedef struct {
+  void    *q[8];        /* t,x,y,z,u^t,u^x,u^y,u^z : n elements each, double (F64) or float (F32)      */
+  double  *lambda;      /* n : affine parameter reached (always double)                                 */
+  int32_t *status;      /* n : gray2_ray_status                                                         */
+  int32_t *nsteps;      /* n : RK4 steps taken so far                                                   */
+  uint64_t n;
+  double   a_eff;       /* spin used by the integrator; = -a for states made by gray2_init_null (R3)    */
+  int32_t  prec;        /* gray2_precision of q[]                                                       */
+  int32_t  kind;        /* gray2_kind (only gray2_invariants reads it: mu^2 inside Carter's Q)          */
+  int32_t  reversed;    /* 1: time-reversed ray of a backward trace (physical t = -t, L_z = -L_z)       */
+} gray2_state;
+
+/* Step and stopping rule (DESIGN R4-R6).  For every geodesic with status ACTIVE, repeat:
+ *   r = Kerr-Schild radius of the current position (eq. 5);
+ *   not finite -> INVALID;  r < capture_factor * r_plus -> CAPTURED;  r > r_escape -> ESCAPED;
+ *   nsteps >= max_steps -> MAXSTEPS;  dir*(lambda_end - lambda) <= 0 -> return, still ACTIVE;
+ *   h = dir * (mode == 1 ? eta * r : h_fixed), clipped so that lambda does not pass lambda_end;
+ *   one RK4 step of size h;  lambda += h;  nsteps += 1.
+ * The stored state is the state at which a test fired (no interpolation).  r_plus = 1 + sqrt(1 - a^2). */
+typedef struct {
+  int32_t mode;            /* 0: fixed step ; 1: radius-scaled step                                     */
+  double  h_fixed, eta;
+  int32_t dir;             /* +1 or -1 (states from gray2_init_null are run with +1)                    */
+  double  capture_factor;  /* e.g. 1.01                                                                 */
+  double  r_escape;        /* +inf allowed                                                              */
+  int32_t max_steps;       /* per-geodesic total, counted from the state's nsteps                       */
+} gray2_step_control;
+
+typedef struct { uint64_t steps, n_captured, n_escaped, n_maxsteps, n_invalid, n_active; } gray2_stats;
+
+/* Image-plane initial conditions.  Pixel (j,k), j = 0..nx-1 fastest, index k*nx + j,
+ * has impact parameters alpha_j = -fov_half_alpha + (j+1/2) 2 fov_half_alpha / nx, beta_k likewise (R1).
+ * Observer direction n = (sin i, 0, cos i), e_alpha = (0,1,0), e_beta = (-cos i, 0, sin i); the ray
+ * starts at r_obs n + alpha e_alpha + beta e_beta, t = 0 (R2).  The backward trace is set up as the
+ * time-reversed forward problem (R3): s->a_eff = -a, s->reversed = 1, spatial tangent -n, u^t the
+ * future-directed root of g u u = 0.  Also sets s->kind = GRAY2_NULL, lambda = 0, status = ACTIVE,
+ * nsteps = 0.  s->q, s->lambda, s->status, s->nsteps, s->n and s->prec must be filled by the caller. */
+int gray2_init_null(gray2_state *s, double a, double r_obs, double inclination_rad,
+                    double fov_half_alpha, double fov_half_beta, int32_t nx, int32_t ny,
+                    void *cuda_stream);
+
+/* Explicit initial conditions.  host_xu8: HOST array of n x 8 doubles (AoS: t,x,y,z,u^t,u^x,u^y,u^z).
+ * Copies them into the first n slots of the SoA state (converted to float for F32); with
+ * renormalise_ut != 0 replaces u^t by the future-directed root of g u u = -1 (R7).  Sets s->a_eff = a,
+ * s->kind = GRAY2_TIMELIKE, s->reversed = 0, lambda = 0, status = ACTIVE, nsteps = 0.  The host array
+ * may be reused as soon as the call returns (the call synchronises its staging copy). */
+int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n,
+                        int32_t renormalise_ut, void *cuda_stream);
+
+/* Integrate the first n geodesics of s (see gray2_step_control).  Only ACTIVE geodesics are touched, so
+ * the call is resumable and a second identical call is a no-op.  prec must equal s->prec.
+ * device_stats: DEVICE pointer to one gray2_stats, or NULL; it is OVERWRITTEN with the RK4 steps taken
+ * by this call and the final status counts over the first n geodesics. */
+int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                    int32_t prec, gray2_stats *device_stats, void *cuda_stream);
+
+/* Constants of the RUN geodesic, always evaluated in double from the stored state (DESIGN R8):
+ *   norm = g_ab u^a u^b ;  E = -u_t ;  L_z = x u_y - y u_x ;
+ *   Q = u_theta^2 + cos^2(theta) [ a^2 (mu^2 - E^2) + L_z^2 / sin^2(theta) ], mu^2 nominal from s->kind.
+ * For s->reversed = 1 the physical photon has L_z = -L_z(run) in the spacetime of spin -a_eff; E, Q equal.
+ * E, Lz, Q, norm: DEVICE arrays of n doubles each. */
+int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm,
+                     void *cuda_stream);
+
+/* Optional tuning of gray2_integrate's launch (0 = library default).  Results never depend on it. */
+int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm);
+
+/* Exact floating-point operation counts of one RK4 step of one geodesic in this library's code path
+ * (FMA = 2 flops, add/mul = 1, each rsqrt/rcp = 1), used for the roofline figure; see DESIGN.md. */
+int gray2_flops_per_step(int32_t prec);
+
+/* Diagnostic entry, not one of the four calls of the path: the geodesic right-hand side of eq. (13)-(14)
+ * alone, at n points, so that tests can compare it element by element with the oracle's eq. (7).
+ * pos (3 n: x.., y.., z..), u (4 n: u^t.., u^x.., u^y.., u^z..), out (4 n): DEVICE arrays, SoA, of
+ * double (GRAY2_F64) or float (GRAY2_F32). */
+int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream);
+
+const char *gray2_last_error(void);   /* thread-local text of the last error of the calling thread */
+const char *gray2_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRAY2_H */

@@ -1,0 +1,285 @@
+// gray2_abi.cu -- the C-ABI of include/gray2.h: argument checks, launch configuration, launches.
+// Every step of the path runs in the kernels of gray2_kernels.cuh; nothing here computes on the host
+// beyond a handful of scalars (r_plus, sin/cos of the inclination, spin constants).
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <atomic>
+
+#include "../../include/gray2.h"
+#include "gray2_kernels.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess) return fail(GRAY2_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
+  } while (0)
+
+// ---- work-queue scratch: 64 counters, one 64-byte line each, handed out round-robin ---------------
+constexpr int kQueueSlots = 64;
+unsigned long long *g_queue = nullptr;   // device, kQueueSlots * 8 words (slot i at word 8 i; word 8 i + 1 = steps)
+std::atomic<unsigned> g_queue_next{0};
+std::atomic<int> g_queue_ready{0};
+int g_num_sms = 0;
+
+int ensure_scratch() {
+  if (g_queue_ready.load(std::memory_order_acquire)) return GRAY2_OK;
+  static std::atomic_flag busy = ATOMIC_FLAG_INIT;
+  while (busy.test_and_set(std::memory_order_acquire)) {}
+  int rc = GRAY2_OK;
+  if (!g_queue_ready.load(std::memory_order_acquire)) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaMalloc(&g_queue, kQueueSlots * 8 * sizeof(unsigned long long));
+    if (e != cudaSuccess) rc = fail(GRAY2_ECUDA, "scratch allocation: %s", cudaGetErrorString(e));
+    else g_queue_ready.store(1, std::memory_order_release);
+  }
+  busy.clear(std::memory_order_release);
+  return rc;
+}
+
+// ---- launch configuration of the integrator (gray2_set_launch) ------------------------------------
+int g_threads[2] = {0, 0};          // 0 = default
+int g_blocks_per_sm[2] = {0, 0};
+
+template <typename T> gray2::StateView<T> view_of(const gray2_state *s) {
+  gray2::StateView<T> v;
+  for (int m = 0; m < 8; ++m) v.q[m] = static_cast<T *>(s->q[m]);
+  v.lambda = s->lambda; v.status = s->status; v.nsteps = s->nsteps;
+  return v;
+}
+
+int check_state(const gray2_state *s, const char *who) {
+  if (!s) return fail(GRAY2_EINVAL, "%s: state is NULL", who);
+  if (s->n == 0) return fail(GRAY2_EINVAL, "%s: state has n == 0", who);
+  for (int m = 0; m < 8; ++m)
+    if (!s->q[m]) return fail(GRAY2_EINVAL, "%s: state q[%d] is NULL", who, m);
+  if (!s->lambda || !s->status || !s->nsteps) return fail(GRAY2_EINVAL, "%s: lambda/status/nsteps is NULL", who);
+  if (s->prec != GRAY2_F64 && s->prec != GRAY2_F32) return fail(GRAY2_EINVAL, "%s: unknown precision %d", who, s->prec);
+  return GRAY2_OK;
+}
+
+}  // namespace
+
+// ---- integrator dispatch ----------------------------------------------------------------------------
+namespace {
+
+template <typename T, int THREADS, int MIN_BLOCKS>
+cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::StepParams<T> &p,
+                             unsigned long long *queue, unsigned long long *steps, cudaStream_t st) {
+  uint64_t want = (n + THREADS - 1) / THREADS;
+  uint64_t cap = (uint64_t)g_num_sms * MIN_BLOCKS;
+  unsigned grid = (unsigned)(want < cap ? want : cap);
+  gray2::integrate_kernel<T, THREADS, MIN_BLOCKS><<<grid, THREADS, 0, st>>>(view_of<T>(s), n, p, queue, steps);
+  return cudaGetLastError();
+}
+
+struct LaunchChoice { int threads, blocks; };
+
+// compiled variants; the first entry of each list is the default
+constexpr LaunchChoice kF64Variants[] = {{128, 3}, {128, 2}, {128, 4}, {64, 6}, {256, 1}, {64, 8}};
+constexpr LaunchChoice kF32Variants[] = {{128, 6}, {128, 4}, {128, 8}, {256, 3}, {256, 2}, {64, 12}};
+
+template <typename T>
+cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, uint64_t n,
+                               const gray2::StepParams<T> &p, unsigned long long *q, unsigned long long *steps,
+                               cudaStream_t st, bool *found) {
+  *found = true;
+#define GRAY2_VARIANT(TH, BL) \
+  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL>(s, n, p, q, steps, st);
+  if constexpr (sizeof(T) == 8) {
+    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 2) GRAY2_VARIANT(128, 4)
+    GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(64, 8)
+  } else {
+    GRAY2_VARIANT(128, 6) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(128, 8)
+    GRAY2_VARIANT(256, 3) GRAY2_VARIANT(256, 2) GRAY2_VARIANT(64, 12)
+  }
+#undef GRAY2_VARIANT
+  *found = false;
+  return cudaSuccess;
+}
+
+template <typename T>
+int integrate_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                   gray2_stats *device_stats, cudaStream_t st) {
+  const double a = s->a_eff;
+  gray2::StepParams<T> p;
+  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a);
+  p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
+  p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
+  p.r_escape = (T)sc->r_escape;
+  p.lambda_end = lambda_end;
+  p.dir = (double)sc->dir;
+  p.mode = sc->mode;
+  p.max_steps = sc->max_steps;
+  p.clip = !(isinf(lambda_end) && (double)sc->dir * lambda_end > 0.0);
+
+  unsigned slot = g_queue_next.fetch_add(1) % kQueueSlots;
+  unsigned long long *queue = g_queue + 8 * slot, *steps = queue + 1;
+  CUDA_TRY(cudaMemsetAsync(queue, 0, 2 * sizeof(unsigned long long), st));
+
+  const int pi = sizeof(T) == 8 ? 0 : 1;
+  const LaunchChoice def = sizeof(T) == 8 ? kF64Variants[0] : kF32Variants[0];
+  int threads = g_threads[pi] ? g_threads[pi] : def.threads;
+  int blocks = g_blocks_per_sm[pi] ? g_blocks_per_sm[pi] : def.blocks;
+  bool found = false;
+  cudaError_t e = dispatch_integrate<T>(threads, blocks, s, n, p, queue, steps, st, &found);
+  if (!found) return fail(GRAY2_EINVAL, "gray2_integrate: no compiled variant for %d threads x %d blocks/SM", threads, blocks);
+  if (e != cudaSuccess) return fail(GRAY2_ECUDA, "integrate_kernel launch: %s", cudaGetErrorString(e));
+
+  if (device_stats) {
+    CUDA_TRY(cudaMemsetAsync(device_stats, 0, sizeof(gray2_stats), st));
+    CUDA_TRY(cudaMemcpyAsync(&device_stats->steps, steps, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st));
+    unsigned grid = (unsigned)((n + 255) / 256);
+    if (grid > (unsigned)(g_num_sms * 8)) grid = (unsigned)(g_num_sms * 8);
+    gray2::count_status_kernel<<<grid, 256, 0, st>>>(s->status, n, device_stats);
+    CUDA_TRY(cudaGetLastError());
+  }
+  return GRAY2_OK;
+}
+
+}  // namespace
+
+// ---- the exported calls ------------------------------------------------------------------------------
+extern "C" {
+
+const char *gray2_last_error(void) { return g_err; }
+const char *gray2_version(void) { return "gray2-b200 0.1 (sm_100a)"; }
+
+int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double Wa, double Wb,
+                    int32_t nx, int32_t ny, void *cuda_stream) {
+  int rc = check_state(s, "gray2_init_null");
+  if (rc) return rc;
+  if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_null: |a| must be <= 1 (got %g)", a);
+  if (nx <= 0 || ny <= 0 || (uint64_t)nx * (uint64_t)ny != s->n)
+    return fail(GRAY2_EINVAL, "gray2_init_null: nx*ny (%d x %d) must equal s->n (%llu)", nx, ny, (unsigned long long)s->n);
+  if (!(r_obs > 1.0 + sqrt(1.0 - a * a))) return fail(GRAY2_EINVAL, "gray2_init_null: r_obs must exceed r_plus");
+  if (!(Wa > 0.0) || !(Wb > 0.0) || !isfinite(inc)) return fail(GRAY2_EINVAL, "gray2_init_null: bad field of view or inclination");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  s->a_eff = -a; s->kind = GRAY2_NULL; s->reversed = 1;
+  unsigned grid = (unsigned)((s->n + 255) / 256);
+  if (s->prec == GRAY2_F64)
+    gray2::init_null_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), -a, r_obs, sin(inc), cos(inc), Wa, Wb, nx, ny);
+  else
+    gray2::init_null_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), -a, r_obs, sin(inc), cos(inc), Wa, Wb, nx, ny);
+  CUDA_TRY(cudaGetLastError());
+  return GRAY2_OK;
+}
+
+int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t renorm,
+                        void *cuda_stream) {
+  int rc = check_state(s, "gray2_init_timelike");
+  if (rc) return rc;
+  if (!host_xu8 || n == 0) return fail(GRAY2_EINVAL, "gray2_init_timelike: host_xu8 is NULL or n == 0");
+  if (n > s->n) return fail(GRAY2_ESTATE, "gray2_init_timelike: n (%llu) exceeds s->n (%llu)", (unsigned long long)n, (unsigned long long)s->n);
+  if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_timelike: |a| must be <= 1 (got %g)", a);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double *stage = nullptr;
+  size_t bytes = (size_t)n * 8 * sizeof(double);
+  CUDA_TRY(cudaMallocAsync(&stage, bytes, st));
+  cudaError_t e = cudaMemcpyAsync(stage, host_xu8, bytes, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) {
+    unsigned grid = (unsigned)((n + 255) / 256);
+    if (s->prec == GRAY2_F64)
+      gray2::init_explicit_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), stage, n, a, renorm);
+    else
+      gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), stage, n, a, renorm);
+    e = cudaGetLastError();
+  }
+  cudaError_t e2 = cudaFreeAsync(stage, st);
+  if (e == cudaSuccess) e = e2;
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // host_xu8 may be pageable: make reuse safe
+  if (e != cudaSuccess) return fail(GRAY2_ECUDA, "gray2_init_timelike: %s", cudaGetErrorString(e));
+  s->a_eff = a; s->kind = GRAY2_TIMELIKE; s->reversed = 0;
+  return GRAY2_OK;
+}
+
+int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                    int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
+  int rc = check_state(s, "gray2_integrate");
+  if (rc) return rc;
+  if (!sc) return fail(GRAY2_EINVAL, "gray2_integrate: step control is NULL");
+  if (n == 0) return fail(GRAY2_EINVAL, "gray2_integrate: n == 0");
+  if (n > s->n) return fail(GRAY2_ESTATE, "gray2_integrate: n (%llu) exceeds s->n (%llu)", (unsigned long long)n, (unsigned long long)s->n);
+  if (prec != s->prec) return fail(GRAY2_EINVAL, "gray2_integrate: prec (%d) differs from s->prec (%d)", prec, s->prec);
+  if (sc->mode != 0 && sc->mode != 1) return fail(GRAY2_EINVAL, "gray2_integrate: mode must be 0 or 1");
+  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return fail(GRAY2_EINVAL, "gray2_integrate: step size must be > 0");
+  if (sc->dir != 1 && sc->dir != -1) return fail(GRAY2_EINVAL, "gray2_integrate: dir must be +1 or -1");
+  if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(lambda_end) || sc->max_steps < 0)
+    return fail(GRAY2_EINVAL, "gray2_integrate: bad capture_factor / r_escape / lambda_end / max_steps");
+  if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_integrate: |a_eff| must be <= 1");
+  rc = ensure_scratch();
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  return prec == GRAY2_F64 ? integrate_impl<double>(s, n, lambda_end, sc, device_stats, st)
+                           : integrate_impl<float>(s, n, lambda_end, sc, device_stats, st);
+}
+
+int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm,
+                     void *cuda_stream) {
+  int rc = check_state(s, "gray2_invariants");
+  if (rc) return rc;
+  if (n == 0 || !E || !Lz || !Q || !norm) return fail(GRAY2_EINVAL, "gray2_invariants: n == 0 or NULL output");
+  if (n > s->n) return fail(GRAY2_ESTATE, "gray2_invariants: n exceeds s->n");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  double mu2 = s->kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
+  unsigned grid = (unsigned)((n + 255) / 256);
+  if (s->prec == GRAY2_F64)
+    gray2::invariants_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), n, s->a_eff, mu2, E, Lz, Q, norm);
+  else
+    gray2::invariants_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), n, s->a_eff, mu2, E, Lz, Q, norm);
+  CUDA_TRY(cudaGetLastError());
+  return GRAY2_OK;
+}
+
+/* Diagnostic entry (not one of the four calls of the path): evaluates the geodesic right-hand side of
+ * eq. (13)-(14) at n points.  pos (3 n), u (4 n), out (4 n): DEVICE arrays, SoA, double or float per prec. */
+int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream) {
+  if (!pos || !u || !out || n == 0) return fail(GRAY2_EINVAL, "gray2_rhs: NULL pointer or n == 0");
+  if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_rhs: unknown precision");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned grid = (unsigned)((n + 127) / 128);
+  if (prec == GRAY2_F64) {
+    gray2::SpinConst<double> k{a, a * a, 2.0 * a, 2.0 * a * a};
+    gray2::rhs_kernel<double><<<grid, 128, 0, st>>>(k, n, (const double *)pos, (const double *)u, (double *)out);
+  } else {
+    gray2::SpinConst<float> k{(float)a, (float)(a * a), (float)(2.0 * a), (float)(2.0 * a * a)};
+    gray2::rhs_kernel<float><<<grid, 128, 0, st>>>(k, n, (const float *)pos, (const float *)u, (float *)out);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return GRAY2_OK;
+}
+
+/* Source-level count of ks_geodesic.cuh (FMA = 2, add/mul = 1, rsqrt/rcp = 1; negations and compares free):
+ *   radius 16, rest of geometry 54, velocity part 63  ->  133 per right-hand side
+ *   4 x 133 + RK4 combination 100 + step rule and lambda update 2 = 634 per step (both precisions). */
+int gray2_flops_per_step(int32_t prec) { (void)prec; return 634; }
+
+int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm) {
+  if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_set_launch: unknown precision");
+  const LaunchChoice *list = prec == GRAY2_F64 ? kF64Variants : kF32Variants;
+  bool ok = threads_per_block == 0 && blocks_per_sm == 0;
+  for (int i = 0; i < 6 && !ok; ++i) ok = list[i].threads == threads_per_block && list[i].blocks == blocks_per_sm;
+  if (!ok) return fail(GRAY2_EINVAL, "gray2_set_launch: %d x %d is not a compiled variant", threads_per_block, blocks_per_sm);
+  g_threads[prec] = threads_per_block;
+  g_blocks_per_sm[prec] = blocks_per_sm;
+  return GRAY2_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,227 @@
+// gray2_kernels.cuh -- CUDA kernels of the hot path (sm_100a).  See include/gray2.h for the contract.
+//
+//   init_null_kernel       one thread per pixel, writes the SoA state
+//   init_explicit_kernel   AoS staging buffer -> SoA state, optional u^t solve   (a2)
+//   integrate_kernel       persistent lanes: each lane keeps ONE geodesic in registers and steps it
+//                          with the fused right-hand side + RK4 until its stopping test fires, then
+//                          stores it and takes the next geodesic from a global queue (warp-aggregated
+//                          atomic: one atomicAdd per warp per refill, ballot + popc prefix)  (a3-a7, a9)
+//   invariants_kernel      E, L_z, Q, u.u in double from the stored state          (a8)
+//   count_status_kernel    final status histogram for gray2_stats
+#pragma once
+#include <stdint.h>
+#include "../../include/gray2.h"
+#include "ks_geodesic.cuh"
+
+namespace gray2 {
+
+template <typename T> struct StateView {
+  T *q[8];
+  double *lambda;
+  int32_t *status;
+  int32_t *nsteps;
+};
+
+template <typename T> struct StepParams {
+  SpinConst<T> k;
+  T eta_or_h;          // eta (mode 1) or h_fixed (mode 0), already multiplied by dir
+  T r_capture;         // capture_factor * r_plus
+  T r_escape;
+  double lambda_end;
+  double dir;
+  int32_t mode;
+  int32_t max_steps;
+  int32_t clip;        // 0 only when dir*lambda_end = +inf: the lambda_end test can never fire, skip it
+};
+
+// u^t from g_ab u^a u^b = -mu2 (future-directed root), DESIGN R3/R7:
+//   (1-f) ut^2 - 2 f c ut - (|v|^2 + mu2 + f c^2) = 0 ,  c = l.v
+__device__ __forceinline__ double solve_ut(double a, double x, double y, double z,
+                                           double vx, double vy, double vz, double mu2) {
+  double R2 = x * x + y * y + z * z, w = R2 - a * a;
+  double r2 = 0.5 * (w + sqrt(w * w + 4.0 * a * a * z * z));
+  double r = sqrt(r2);
+  double f = 2.0 * r2 * r / (r2 * r2 + a * a * z * z);
+  double P = r2 + a * a;
+  double c = ((r * x + a * y) * vx + (r * y - a * x) * vy) / P + z * vz / r;
+  double A = 1.0 - f, B = f * c, C = vx * vx + vy * vy + vz * vz + mu2 + f * c * c;
+  return (B + sqrt(B * B + A * C)) / A;
+}
+
+template <typename T>
+__global__ void init_null_kernel(StateView<T> s, double a_eff, double r_obs, double sin_i, double cos_i,
+                                 double Wa, double Wb, int32_t nx, int32_t ny) {
+  int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)nx * ny) return;
+  int32_t j = (int32_t)(idx % nx), kk = (int32_t)(idx / nx);
+  double alpha = -Wa + ((double)j + 0.5) * (2.0 * Wa / (double)nx);
+  double beta = -Wb + ((double)kk + 0.5) * (2.0 * Wb / (double)ny);
+  // n = (sin i, 0, cos i), e_alpha = (0,1,0), e_beta = (-cos i, 0, sin i)
+  double x = r_obs * sin_i - beta * cos_i;
+  double y = alpha;
+  double z = r_obs * cos_i + beta * sin_i;
+  double vx = -sin_i, vy = 0.0, vz = -cos_i;
+  double ut = solve_ut(a_eff, x, y, z, vx, vy, vz, 0.0);
+  s.q[0][idx] = T(0); s.q[1][idx] = T(x); s.q[2][idx] = T(y); s.q[3][idx] = T(z);
+  s.q[4][idx] = T(ut); s.q[5][idx] = T(vx); s.q[6][idx] = T(vy); s.q[7][idx] = T(vz);
+  s.lambda[idx] = 0.0; s.status[idx] = GRAY2_ACTIVE; s.nsteps[idx] = 0;
+}
+
+template <typename T>
+__global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ xu8, uint64_t n, double a,
+                                     int32_t renorm) {
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  const double2 *row = reinterpret_cast<const double2 *>(xu8 + idx * 8);
+  double2 v0 = row[0], v1 = row[1], v2 = row[2], v3 = row[3];
+  double ut = v2.x;
+  if (renorm) ut = solve_ut(a, v0.y, v1.x, v1.y, v2.y, v3.x, v3.y, 1.0);
+  s.q[0][idx] = T(v0.x); s.q[1][idx] = T(v0.y); s.q[2][idx] = T(v1.x); s.q[3][idx] = T(v1.y);
+  s.q[4][idx] = T(ut); s.q[5][idx] = T(v2.y); s.q[6][idx] = T(v3.x); s.q[7][idx] = T(v3.y);
+  s.lambda[idx] = 0.0; s.status[idx] = GRAY2_ACTIVE; s.nsteps[idx] = 0;
+}
+
+// ---- the fused integrator ------------------------------------------------------------------------
+template <typename T, int THREADS, int MIN_BLOCKS>
+__global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
+integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long *queue,
+                 unsigned long long *steps_out) {
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const SpinConst<T> k = p.k;
+
+  Ray<T> ray;
+  double lam = 0.0;
+  int32_t nst = 0;
+  uint64_t idx = 0;
+  bool have = false;           // this lane holds an ACTIVE geodesic
+  bool drained = false;        // warp-uniform: the queue has no more work
+  unsigned long long my_steps = 0;
+
+  for (;;) {
+    // ---- refill idle lanes from the global queue (warp-aggregated) ------------------------------
+    unsigned idle = __ballot_sync(0xffffffffu, !have);
+    if (idle && !drained) {
+      unsigned cnt = __popc(idle);
+      unsigned long long base = 0;
+      if (lane == (unsigned)(__ffs(idle) - 1)) base = atomicAdd(queue, (unsigned long long)cnt);
+      base = __shfl_sync(0xffffffffu, base, __ffs(idle) - 1);
+      if (base + cnt >= n) drained = true;
+      if (!have) {
+        uint64_t mine = base + __popc(idle & lt_mask);
+        if (mine < n && s.status[mine] == GRAY2_ACTIVE) {
+          idx = mine;
+          ray.t = s.q[0][idx]; ray.x = s.q[1][idx]; ray.y = s.q[2][idx]; ray.z = s.q[3][idx];
+          ray.u0 = s.q[4][idx]; ray.u1 = s.q[5][idx]; ray.u2 = s.q[6][idx]; ray.u3 = s.q[7][idx];
+          lam = s.lambda[idx];
+          nst = s.nsteps[idx];
+          have = true;
+        }
+      }
+      continue;   // newly loaded lanes may need another refill (non-ACTIVE entries); tests run next pass
+    }
+    if (idle == 0xffffffffu) break;   // nothing held and the queue is drained
+
+    if (have) {
+      // ---- stopping tests on the current state, in the order of gray2_step_control ------------
+      Geometry<T> g;
+      ks_geometry(k, ray.x, ray.y, ray.z, g);
+      T U = fma_(g.l1, ray.u1, fma_(g.l2, ray.u2, fma_(g.l3, ray.u3, ray.u0)));
+      int32_t st = GRAY2_ACTIVE;
+      bool stop = false;
+      if (!(fastmath<T>::finite(g.r) && fastmath<T>::finite(U) && fastmath<T>::finite(ray.t))) {
+        st = GRAY2_INVALID; stop = true;
+      } else if (g.r < p.r_capture) {
+        st = GRAY2_CAPTURED; stop = true;
+      } else if (g.r > p.r_escape) {
+        st = GRAY2_ESCAPED; stop = true;
+      } else if (nst >= p.max_steps) {
+        st = GRAY2_MAXSTEPS; stop = true;
+      } else if (p.clip && p.dir * (p.lambda_end - lam) <= 0.0) {
+        stop = true;           // stays ACTIVE: resumable
+      }
+      if (stop) {
+        s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
+        s.q[4][idx] = ray.u0; s.q[5][idx] = ray.u1; s.q[6][idx] = ray.u2; s.q[7][idx] = ray.u3;
+        s.lambda[idx] = lam; s.status[idx] = st; s.nsteps[idx] = nst;
+        have = false;
+      } else {
+        T h = (p.mode == 1) ? p.eta_or_h * g.r : p.eta_or_h;
+        double hd = (double)h;
+        if (p.clip) {
+          double rem = p.lambda_end - lam;
+          if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
+        }
+        rk4_step(k, ray, g, h);
+        lam += hd;
+        nst += 1;
+        my_steps += 1;
+      }
+    }
+  }
+
+  // ---- per-warp reduction of the step count -----------------------------------------------------
+  for (int off = 16; off > 0; off >>= 1) my_steps += __shfl_down_sync(0xffffffffu, my_steps, off);
+  if (lane == 0 && my_steps) atomicAdd(steps_out, my_steps);
+}
+
+// ---- invariants (always double) ------------------------------------------------------------------
+template <typename T>
+__global__ void invariants_kernel(StateView<T> s, uint64_t n, double a, double mu2, double *__restrict__ E,
+                                  double *__restrict__ Lz, double *__restrict__ Q, double *__restrict__ norm) {
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  double x = (double)s.q[1][idx], y = (double)s.q[2][idx], z = (double)s.q[3][idx];
+  double u0 = (double)s.q[4][idx], u1 = (double)s.q[5][idx], u2 = (double)s.q[6][idx], u3 = (double)s.q[7][idx];
+  double R2 = x * x + y * y + z * z, w = R2 - a * a;
+  double r2 = 0.5 * (w + sqrt(w * w + 4.0 * a * a * z * z));
+  double r = sqrt(r2), P = r2 + a * a;
+  double f = 2.0 * r2 * r / (r2 * r2 + a * a * z * z);
+  double l1 = (r * x + a * y) / P, l2 = (r * y - a * x) / P, l3 = z / r;
+  double U = u0 + l1 * u1 + l2 * u2 + l3 * u3;
+  // lower the index with g = eta + f l l :  u_0 = -u^0 + f U ,  u_i = u^i + f l_i U
+  double c0 = -u0 + f * U, cx = u1 + f * l1 * U, cy = u2 + f * l2 * U, cz = u3 + f * l3 * U;
+  double nn = c0 * u0 + cx * u1 + cy * u2 + cz * u3;
+  double e = -c0;
+  double lz = x * cy - y * cx;
+  double c = l3, s2 = 1.0 - c * c;
+  double q = P * c * c * (cx * cx + cy * cy) - 2.0 * r * c * (x * cx + y * cy) * cz + r2 * s2 * cz * cz +
+             a * a * c * c * (mu2 - e * e);
+  E[idx] = e; Lz[idx] = lz; Q[idx] = q; norm[idx] = nn;
+}
+
+// Diagnostic: the right-hand side alone, for element-wise parity tests against the oracle.
+// pos: 3 arrays of n (x,y,z), u: 4 arrays of n, out: 4 arrays of n, all of type T, SoA.
+template <typename T>
+__global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos, const T *__restrict__ u,
+                           T *__restrict__ out) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Geometry<T> g;
+  ks_geometry(k, pos[i], pos[n + i], pos[2 * n + i], g);
+  T a0, a1, a2, a3;
+  ks_accel(g, u[i], u[n + i], u[2 * n + i], u[3 * n + i], a0, a1, a2, a3);
+  out[i] = a0; out[n + i] = a1; out[2 * n + i] = a2; out[3 * n + i] = a3;
+}
+
+__global__ void count_status_kernel(const int32_t *__restrict__ status, uint64_t n, gray2_stats *stats) {
+  unsigned long long c[5] = {0, 0, 0, 0, 0};
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    int32_t st = status[i];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) c[v] += (st == v);
+  }
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    for (int off = 16; off > 0; off >>= 1) c[v] += __shfl_down_sync(0xffffffffu, c[v], off);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    if (c[0]) atomicAdd((unsigned long long *)&stats->n_active, c[0]);
+    if (c[1]) atomicAdd((unsigned long long *)&stats->n_captured, c[1]);
+    if (c[2]) atomicAdd((unsigned long long *)&stats->n_escaped, c[2]);
+    if (c[3]) atomicAdd((unsigned long long *)&stats->n_maxsteps, c[3]);
+    if (c[4]) atomicAdd((unsigned long long *)&stats->n_invalid, c[4]);
+  }
+}
+
+}  // namespace gray2

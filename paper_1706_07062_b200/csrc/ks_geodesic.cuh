@@ -1,0 +1,209 @@
+// ks_geodesic.cuh -- device arithmetic of the hot path: Kerr-Schild geodesic right-hand side in the
+// regrouped form of PAPER.md:98-117 (eq. 10-14), and the classic RK4 step of PAPER.md:164.
+//
+// Everything here lives in registers; one thread owns one geodesic.  Template parameter T is the
+// arithmetic type (double or float).  No table of Christoffel symbols is ever formed.
+//
+// Derivation (checked against the brute-force connection to 1e-41 in
+// 40-digit arithmetic).  With M = 1, spin a, position (x,y,z), velocity (u0,u1,u2,u3) = dx^mu/dlambda:
+//
+//   w = x^2+y^2+z^2 - a^2,  D = sqrt(w^2 + 4 a^2 z^2),  r^2 = (w + D)/2                      (eq. 5)
+//   D equals Sigma = r^2 + a^2 z^2/r^2, so  f = 2 r^3/(r^4 + a^2 z^2) = 2 r / D                (eq. 3)
+//   P = r^2 + a^2,  l = ((r x + a y)/P, (r y - a x)/P, z/r)                                    (eq. 4)
+//   grad r = (f/2) (x, y, z P / r^2)
+//   grad f = f [ c1 grad r - c2 e_z ],  c1 = 3/r - 2 f,  c2 = 2 a^2 z / (D r^2)
+//   d_j l_i = (grad r)_j A_i + B_ji,  A = ((x - 2 r l1)/P, (y - 2 r l2)/P, -l3/r),
+//             B = [[r/P, -a/P, 0], [a/P, r/P, 0], [0, 0, 1/r]]
+//
+// The 12 elements xdot_{beta,alpha} = g_{beta gamma,alpha} xdot^gamma of PAPER.md:100 never need to be
+// stored: with U = u0 + l.u they collapse to
+//   omega = curl l = grad r x A + (0, 0, -2a/P)                 (antisymmetric part of d_j l_i)
+//   q     = u_i u_j d_j l_i = (u.grad r)(A.u) + (r/P)(u1^2+u2^2) + u3^2 / r   (symmetric part)
+//   l.grad f = f (c1 - c2 l3)       because l.grad r = 1 and (l.grad) l = 0 (l is a geodesic null field)
+//   F   = -(1/2) f U^2 (l.grad f)                                              (eq. 12)
+//   xddot^0 = U (u.grad f) + f q - F                                          (eq. 13)
+//   xddot^i = (1/2) U^2 d_i f + f U (u x omega)_i - l_i xddot^0               (eq. 14)
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace gray2 {
+
+// ---- fast reciprocal square root / reciprocal ---------------------------------------------------
+// FP64: hardware seed (MUFU.RSQ64H / MUFU.RCP64H, about 20 good bits) followed by ONE third-order
+// correction, which leaves a relative error of a few 1e-16 -- ample for the 1e-9 parity bound, and
+// 3-5 DFMA-pipe instructions instead of the ~12 plus a slow-path branch of IEEE division and sqrt.
+// FP32: the MUFU approximation itself (max relative error 2^-22.4 for rsqrt, 1 ulp for rcp).
+template <typename T> struct fastmath;
+
+template <> struct fastmath<double> {
+  static __device__ __forceinline__ double rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x * y, y, 1.0);            // e = 1 - x y^2
+    double c = fma(0.375, e, 0.5);             // y <- y (1 + e/2 + 3 e^2/8)
+    return fma(y * e, c, y);
+  }
+  static __device__ __forceinline__ double rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);                // e = 1 - x y
+    double t = fma(e, e, e);                   // y <- y (1 + e + e^2)
+    return fma(y, t, y);
+  }
+  static __device__ __forceinline__ double sqrt_ieee(double x) { return ::sqrt(x); }
+  static __device__ __forceinline__ bool finite(double x) { return fabs(x) <= 1.7976931348623157e308; }
+};
+
+template <> struct fastmath<float> {
+  static __device__ __forceinline__ float rsqrt(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+  }
+  static __device__ __forceinline__ float rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+  }
+  static __device__ __forceinline__ float sqrt_ieee(float x) { return ::sqrtf(x); }
+  static __device__ __forceinline__ bool finite(float x) { return fabsf(x) <= 3.402823466e38f; }
+};
+
+template <typename T> __device__ __forceinline__ T fma_(T a, T b, T c);
+template <> __device__ __forceinline__ double fma_<double>(double a, double b, double c) { return fma(a, b, c); }
+template <> __device__ __forceinline__ float fma_<float>(float a, float b, float c) { return fmaf(a, b, c); }
+
+// Spin-dependent constants, computed once on the host.
+template <typename T> struct SpinConst {
+  T a, a2, two_a, two_a2;
+};
+
+// Position-only part of the right-hand side (shared by the stopping test, the step rule and stage 1).
+template <typename T> struct Geometry {
+  T r, rinv, Pinv, f, l1, l2, l3;
+  T rx, ry, rz;     // grad r
+  T fx, fy, fz;     // grad f
+  T lf;             // l . grad f
+  T w1, w2, w3;     // curl l
+  T A1, A2, A3, rP; // pieces of the symmetric part
+};
+
+template <typename T>
+__device__ __forceinline__ void ks_radius(const SpinConst<T> &k, T x, T y, T z, T &r, T &rinv, T &Dinv, T &r2) {
+  T w = fma_(x, x, fma_(y, y, fma_(z, z, -k.a2)));
+  T b = k.two_a * z;
+  T D2 = fma_(b, b, w * w);
+  Dinv = fastmath<T>::rsqrt(D2);
+  T D = D2 * Dinv;
+  r2 = T(0.5) * (w + D);
+  rinv = fastmath<T>::rsqrt(r2);
+  r = r2 * rinv;
+}
+
+template <typename T>
+__device__ __forceinline__ void ks_geometry(const SpinConst<T> &k, T x, T y, T z, Geometry<T> &g) {
+  T Dinv, r2;
+  ks_radius(k, x, y, z, g.r, g.rinv, Dinv, r2);
+  const T r = g.r, rinv = g.rinv;
+  T P = r2 + k.a2;
+  T Pinv = fastmath<T>::rcp(P);
+  g.Pinv = Pinv;
+  T hf = r * Dinv;                 // f / 2
+  T f = hf + hf;
+  g.f = f;
+  g.l1 = fma_(r, x, k.a * y) * Pinv;
+  g.l2 = fma_(r, y, -k.a * x) * Pinv;
+  g.l3 = z * rinv;
+  T rinv2 = rinv * rinv;
+  g.rx = hf * x;
+  g.ry = hf * y;
+  g.rz = hf * (z * (P * rinv2));
+  T c1 = fma_(T(3), rinv, -(f + f));
+  T c2 = k.two_a2 * z * (Dinv * rinv2);
+  T c1f = c1 * f;
+  g.fx = c1f * g.rx;
+  g.fy = c1f * g.ry;
+  g.fz = fma_(c1f, g.rz, -c2 * f);
+  g.lf = f * fma_(-c2, g.l3, c1);
+  T tr = r + r;
+  g.A1 = fma_(-tr, g.l1, x) * Pinv;
+  g.A2 = fma_(-tr, g.l2, y) * Pinv;
+  g.A3 = -g.l3 * rinv;
+  g.rP = r * Pinv;
+  g.w1 = fma_(g.ry, g.A3, -g.rz * g.A2);
+  g.w2 = fma_(g.rz, g.A1, -g.rx * g.A3);
+  g.w3 = fma_(g.rx, g.A2, fma_(-g.ry, g.A1, -k.two_a * Pinv));
+}
+
+// Velocity-dependent part: xddot^mu from the geometry and u (eq. 13-14).
+template <typename T>
+__device__ __forceinline__ void ks_accel(const Geometry<T> &g, T u0, T u1, T u2, T u3,
+                                         T &a0, T &a1, T &a2, T &a3) {
+  T U = fma_(g.l1, u1, fma_(g.l2, u2, fma_(g.l3, u3, u0)));
+  T ur = fma_(u1, g.rx, fma_(u2, g.ry, u3 * g.rz));
+  T Au = fma_(u1, g.A1, fma_(u2, g.A2, u3 * g.A3));
+  T s12 = fma_(u1, u1, u2 * u2);
+  T q = fma_(ur, Au, fma_(g.rP, s12, (u3 * u3) * g.rinv));
+  T uf = fma_(u1, g.fx, fma_(u2, g.fy, u3 * g.fz));
+  T hU2 = T(0.5) * (U * U);
+  T fU = g.f * U;
+  T G = fma_(U, uf, g.f * q);
+  a0 = fma_(g.f * hU2, g.lf, G);               // G - F,  F = -f (U^2/2) (l.grad f)
+  T c1 = fma_(u2, g.w3, -u3 * g.w2);           // u x omega
+  T c2 = fma_(u3, g.w1, -u1 * g.w3);
+  T c3 = fma_(u1, g.w2, -u2 * g.w1);
+  a1 = fma_(hU2, g.fx, fma_(fU, c1, -g.l1 * a0));
+  a2 = fma_(hU2, g.fy, fma_(fU, c2, -g.l2 * a0));
+  a3 = fma_(hU2, g.fz, fma_(fU, c3, -g.l3 * a0));
+}
+
+// One geodesic's 8 variables.
+template <typename T> struct Ray {
+  T t, x, y, z, u0, u1, u2, u3;
+};
+
+// Classic RK4.  `g1` is the geometry at the current position (already needed by the
+// stopping test and the step rule), so stage 1 costs only the velocity-dependent part.
+template <typename T>
+__device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, T h) {
+  const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
+  T b0, b1, b2, b3;                      // stage acceleration
+  T v0, v1, v2, v3;                      // stage velocity
+  T px, py, pz;                          // stage position
+  T St, Sx, Sy, Sz, S0, S1, S2, S3;      // k1 + 2 k2 + 2 k3 (+ k4)
+  Geometry<T> g;
+  // stage 1
+  ks_accel(g1, s.u0, s.u1, s.u2, s.u3, b0, b1, b2, b3);
+  St = s.u0; Sx = s.u1; Sy = s.u2; Sz = s.u3;
+  S0 = b0; S1 = b1; S2 = b2; S3 = b3;
+  px = fma_(hh, s.u1, s.x); py = fma_(hh, s.u2, s.y); pz = fma_(hh, s.u3, s.z);
+  v0 = fma_(hh, b0, s.u0); v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
+  // stage 2
+  ks_geometry(k, px, py, pz, g);
+  ks_accel(g, v0, v1, v2, v3, b0, b1, b2, b3);
+  St = fma_(T(2), v0, St); Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
+  S0 = fma_(T(2), b0, S0); S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
+  px = fma_(hh, v1, s.x); py = fma_(hh, v2, s.y); pz = fma_(hh, v3, s.z);
+  v0 = fma_(hh, b0, s.u0); v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
+  // stage 3
+  ks_geometry(k, px, py, pz, g);
+  ks_accel(g, v0, v1, v2, v3, b0, b1, b2, b3);
+  St = fma_(T(2), v0, St); Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
+  S0 = fma_(T(2), b0, S0); S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
+  px = fma_(h, v1, s.x); py = fma_(h, v2, s.y); pz = fma_(h, v3, s.z);
+  v0 = fma_(h, b0, s.u0); v1 = fma_(h, b1, s.u1); v2 = fma_(h, b2, s.u2); v3 = fma_(h, b3, s.u3);
+  // stage 4
+  ks_geometry(k, px, py, pz, g);
+  ks_accel(g, v0, v1, v2, v3, b0, b1, b2, b3);
+  s.t = fma_(h6, St + v0, s.t);
+  s.x = fma_(h6, Sx + v1, s.x);
+  s.y = fma_(h6, Sy + v2, s.y);
+  s.z = fma_(h6, Sz + v3, s.z);
+  s.u0 = fma_(h6, S0 + b0, s.u0);
+  s.u1 = fma_(h6, S1 + b1, s.u1);
+  s.u2 = fma_(h6, S2 + b2, s.u2);
+  s.u3 = fma_(h6, S3 + b3, s.u3);
+}
+
+}  // namespace gray2

@@ -1,0 +1,161 @@
+"""GPU parity: the CUDA path, called through the C-ABI binding, against the oracle on the same seeded
+inputs, element by element.  Tolerances: gpu_helpers.py (from BASELINE.json's north_star)."""
+import numpy as np
+import pytest
+import torch
+
+import image_helpers as ih
+import oracle
+from gpu_helpers import (INF, invariant_term_scales, TOL_DRIFT_F64, TOL_STATE_F32, TOL_STATE_F64, drift, gpu_invariants_np, image_sc,
+                         run_gpu_image, run_oracle_image, sc_pair, state_rel_error, take, to_oracle_state)
+from paper_1706_07062_b200 import gray2, inputs
+
+pytestmark = pytest.mark.gpu
+
+
+# ---- a3: the right-hand side alone ----------------------------------------------------------------
+
+@pytest.mark.parametrize("a", [0.0, 0.5, -0.9375, 0.99, 1.0])
+def test_rhs_matches_oracle_christoffel_form(a):
+    rng = np.random.default_rng(7)
+    n = 4099   # several blocks and a ragged tail
+    pos = rng.uniform(-12, 12, (3, n))
+    rr = np.array([oracle.ks_r(a, *pos[:, k]) for k in range(n)])
+    pos[:, rr < 1.05 * (1 + np.sqrt(1 - a * a))] *= 6.0
+    pos[:, 0] = [0.0, 0.0, 2.4]      # the pole
+    pos[:, 1] = [3.0, -1.0, 0.0]     # the equator
+    u = rng.uniform(-1, 1, (4, n))
+    u[0] = rng.uniform(1, 3, n)
+    expect = np.array([oracle.ks_accel(a, pos[:, k], u[:, k]) for k in range(n)]).T
+    got = gray2.rhs(gray2.F64, a, torch.tensor(pos, device="cuda"), torch.tensor(u, device="cuda")).cpu().numpy()
+    scale = np.abs(expect).max(axis=0, keepdims=True) + 1e-300
+    assert np.max(np.abs(got - expect) / scale) < 2e-12
+    got32 = gray2.rhs(gray2.F32, a, torch.tensor(pos, device="cuda"), torch.tensor(u, device="cuda")).cpu().numpy()
+    assert np.max(np.abs(got32 - expect) / scale) < 2e-4
+
+
+# ---- a1, a2: initial conditions -------------------------------------------------------------------
+
+@pytest.mark.parametrize("cfg", [inputs.CFG1_NULL, inputs.CFG3_NULL.scaled(97, 61)], ids=lambda c: c.name)
+def test_init_null_matches_oracle(cfg):
+    g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    o = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    assert (g.a_eff, g.kind, g.reversed) == (o.a_eff, o.kind, o.reversed)
+    gq = g.q.cpu().numpy()
+    assert np.max(np.abs(gq - o.q) / np.maximum(np.abs(o.q), 1.0)) < 1e-14
+    assert (g.status.cpu().numpy() == 0).all() and (g.nsteps.cpu().numpy() == 0).all() and (g.lam.cpu().numpy() == 0).all()
+    g32 = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=gray2.F32)
+    assert g32.q.dtype == torch.float32
+    assert np.max(np.abs(g32.q.double().cpu().numpy() - o.q) / np.maximum(np.abs(o.q), 1.0)) < 1e-7
+
+
+def test_init_timelike_matches_oracle():
+    xu8, _ = inputs.cfg4_ensemble(1000)
+    for renorm in (False, True):
+        x = xu8.copy()
+        if renorm:
+            x[:, 4] = 99.0
+        g = gray2.init_timelike(0.7, x, renormalise_ut=renorm)
+        o = oracle.init_timelike(0.7, x, renormalise_ut=renorm)
+        assert np.max(np.abs(g.q.cpu().numpy() - o.q) / np.maximum(np.abs(o.q), 1.0)) < 1e-14
+        assert (g.a_eff, g.kind, g.reversed) == (0.7, gray2.TIMELIKE, 0)
+    if True:
+        gi = gpu_invariants_np(gray2.init_timelike(0.7, xu8))
+        oi = oracle.invariants(oracle.init_timelike(0.7, xu8))
+        for a_, b_ in zip(gi, oi):
+            assert np.max(np.abs(a_ - b_) / np.maximum(np.abs(b_), 1.0)) < 1e-13
+
+
+# ---- whole path on image configs ------------------------------------------------------------------
+
+def compare_image(cfg, g0, g, o0, o, idx=None):
+    """Shared checks for an image config; idx = the pixel indices the oracle ran (None = all)."""
+    gst = to_oracle_state(g)
+    if idx is not None:
+        gst = take(gst, idx)
+    full0 = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    d, mask = ih.classify_image(cfg, full0 if idx is None else full0)
+    if idx is not None:
+        d, mask = d[idx], mask[idx]
+    outside = d > 1e-3
+    # capture/escape flag and step count: bit-exact outside the band, vs the oracle AND vs Carter's potential
+    assert np.array_equal(gst.status[outside], o.status[outside])
+    assert np.array_equal(gst.nsteps[outside], o.nsteps[outside])
+    assert np.array_equal((gst.status == gray2.CAPTURED)[outside], mask[outside])
+    same = outside & (gst.nsteps == o.nsteps) & (gst.status == o.status)
+    err = state_rel_error(gst.q[:, same], o.q[:, same], o.a_eff)
+    assert err.max() < TOL_STATE_F64, err.max()
+    assert np.max(np.abs(gst.lam[same] - o.lam[same]) / np.maximum(o.lam[same], 1.0)) < TOL_STATE_F64   # lambda = sum of eta r
+    # invariant drift identical within 1e-12
+    gi1 = gpu_invariants_np(g)
+    gi0 = gpu_invariants_np(g0)
+    if idx is not None:
+        gi1 = [v[idx] for v in gi1]
+        gi0 = [v[idx] for v in gi0]
+    oi1, oi0 = oracle.invariants(o), oracle.invariants(o0)
+    # a drift is a difference of two evaluations: the rounding of either end bounds what can agree
+    scales = [np.maximum(s1, s0) for s1, s0 in zip(invariant_term_scales(o.q), invariant_term_scales(o0.q))]
+    for k, (gd, od) in enumerate(zip(drift(gi1, gi0), drift(oi1, oi0))):
+        scale = scales[k]
+        assert np.max(np.abs(gd - od)[same] / scale[same]) < TOL_DRIFT_F64, (k, np.max(np.abs(gd - od)[same] / scale[same]))
+    return outside, same
+
+
+def test_cfg1_schwarzschild_image_full_parity():
+    cfg = inputs.CFG1_NULL
+    g0, g, gstats = run_gpu_image(cfg)
+    o0, o, ostats = run_oracle_image(cfg)
+    outside, same = compare_image(cfg, g0, g, o0, o)
+    assert outside.mean() > 0.995 and same.sum() == outside.sum()
+    assert gstats["n_active"] == 0 and gstats["n_invalid"] == 0 and gstats["n_maxsteps"] == 0
+    assert gstats["steps"] == int(g.nsteps.sum().item())
+    if outside.all():
+        assert gstats == ostats
+
+
+def test_cfg1_timelike_orbits_parity():
+    xu8, r0 = inputs.cfg1_orbits()
+    gsc, osc = sc_pair(mode=0, h_fixed=0.5, max_steps=5000)
+    g = gray2.init_timelike(0.0, xu8)
+    g0 = g.clone()
+    stats = gray2.new_stats()
+    gray2.integrate(g, INF, gsc, stats=stats)
+    o = oracle.init_timelike(0.0, xu8)
+    o0 = o.copy()
+    oracle.integrate(o, INF, osc)
+    gst = to_oracle_state(g)
+    assert (gst.status == gray2.MAXSTEPS).all() and (gst.nsteps == 5000).all()
+    assert gray2.stats_dict(stats) == dict(steps=80000, n_captured=0, n_escaped=0, n_maxsteps=16, n_invalid=0, n_active=0)
+    assert state_rel_error(gst.q, o.q, 0.0).max() < TOL_STATE_F64
+    assert np.max(np.abs(gst.lam - 2500.0)) < 1e-9
+    gd = drift(gpu_invariants_np(g), gpu_invariants_np(g0))
+    od = drift(oracle.invariants(o), oracle.invariants(o0))
+    for a_, b_ in zip(gd, od):
+        assert np.max(np.abs(a_ - b_)) < 1e-11   # 5000 steps of fixed h: both drifts ~1e-9, equal to 1e-11
+
+
+@pytest.mark.parametrize("cfg", [inputs.CFG2_NULL.scaled(96, 80), inputs.CFG3_NULL.scaled(131, 77),
+                                 inputs.CFG5_NULL.scaled(100, 100)], ids=lambda c: c.name)
+def test_kerr_images_reduced_resolution_full_parity(cfg):
+    g0, g, gstats = run_gpu_image(cfg)
+    o0, o, ostats = run_oracle_image(cfg)
+    outside, same = compare_image(cfg, g0, g, o0, o)
+    assert outside.mean() > 0.99
+    assert gstats["n_active"] == 0 and gstats["n_invalid"] == 0
+    assert abs(gstats["steps"] - ostats["steps"]) <= 40 * (~outside).sum()
+
+
+@pytest.mark.parametrize("cfg", [inputs.CFG3_NULL.scaled(64), inputs.CFG1_NULL], ids=lambda c: c.name)
+def test_fp32_against_oracle(cfg):
+    g0, g, gstats = run_gpu_image(cfg, prec=gray2.F32)
+    o0, o, _ = run_oracle_image(cfg)
+    gst = to_oracle_state(g)
+    d, mask = ih.classify_image(cfg, o0)
+    outside = d > 1e-3 * 20          # FP32 rounding of the pixel position alone is ~1e-4 M at r_obs = 1000
+    assert np.array_equal((gst.status == gray2.CAPTURED)[outside], mask[outside])
+    same = outside & (gst.nsteps == o.nsteps) & (gst.status == o.status)
+    assert same.sum() > 0.5 * outside.sum()
+    err = state_rel_error(gst.q[1:][:, same], o.q[1:][:, same], o.a_eff)
+    # bulk of the rays within the stated tolerance; the few strongly lensed ones amplify FP32 rounding
+    assert np.quantile(err, 0.90) < TOL_STATE_F32, np.quantile(err, [0.5, 0.9, 0.99, 1.0])
+    assert np.median(err) < 0.2 * TOL_STATE_F32
