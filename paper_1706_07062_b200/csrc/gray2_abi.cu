@@ -271,6 +271,20 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
  *   4 x 133 + RK4 combination 100 + step rule and lambda update 2 = 634 per step (both precisions). */
 int gray2_flops_per_step(int32_t prec) { (void)prec; return 634; }
 
+/* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
+ * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
+ * scratch: DEVICE pointer to at least one element of the precision's type.  Flops = 16*iters*blocks*threads. */
+int gray2_fma_probe(int32_t prec, int32_t blocks, int32_t threads, int32_t iters, void *scratch, void *cuda_stream) {
+  if (!scratch || blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0)
+    return fail(GRAY2_EINVAL, "gray2_fma_probe: bad argument");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (prec == GRAY2_F64) gray2::fma_probe_kernel<double><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
+  else if (prec == GRAY2_F32) gray2::fma_probe_kernel<float><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+  else return fail(GRAY2_EINVAL, "gray2_fma_probe: unknown precision");
+  CUDA_TRY(cudaGetLastError());
+  return GRAY2_OK;
+}
+
 int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm) {
   if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_set_launch: unknown precision");
   const LaunchChoice *list = prec == GRAY2_F64 ? kF64Variants : kF32Variants;

@@ -204,6 +204,22 @@ __global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos
   out[i] = a0; out[n + i] = a1; out[2 * n + i] = a2; out[3 * n + i] = a3;
 }
 
+// Diagnostic: FMA-only probe of the FP64 / FP32 pipe (8 independent chains per thread, registers only).
+// Each thread executes 8 * iters FMAs; the launch's flop count is 2 * 8 * iters * threads.
+template <typename T>
+__global__ void fma_probe_kernel(int iters, T seed, T *__restrict__ out) {
+  T a0 = seed + T(threadIdx.x), a1 = a0 + T(1), a2 = a0 + T(2), a3 = a0 + T(3);
+  T a4 = a0 + T(4), a5 = a0 + T(5), a6 = a0 + T(6), a7 = a0 + T(7);
+  const T m = T(0.999999), c = T(1e-6);
+#pragma unroll 4
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma_(a0, m, c); a1 = fma_(a1, m, c); a2 = fma_(a2, m, c); a3 = fma_(a3, m, c);
+    a4 = fma_(a4, m, c); a5 = fma_(a5, m, c); a6 = fma_(a6, m, c); a7 = fma_(a7, m, c);
+  }
+  T s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == T(-12345.678)) out[0] = s;   // never true; keeps the chains alive
+}
+
 __global__ void count_status_kernel(const int32_t *__restrict__ status, uint64_t n, gray2_stats *stats) {
   unsigned long long c[5] = {0, 0, 0, 0, 0};
   for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
