@@ -272,13 +272,9 @@ def run_gpu(args):
     fma_probe_tflops = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
 
     # ---- reduce over ranks: time = max, work = sum
-    red = torch.tensor([t_step, t_int, t_e2e], dtype=torch.float64, device="cuda")
-    work = torch.tensor([steps_total, e2e_steps], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(red, op=dist.ReduceOp.MAX)
-        dist.all_reduce(work, op=dist.ReduceOp.SUM)
-    t_step, t_int, t_e2e = red.tolist()
-    steps_all, e2e_all = work.tolist()
+    from paper_1706_07062_b200 import multi
+    (t_step, t_int, t_e2e), (steps_all, e2e_all) = multi.reduce_job([t_step, t_int, t_e2e], [steps_total, e2e_steps],
+                                                                    device="cuda")
 
     if rank == 0:
         value = steps_all / t_step

@@ -86,15 +86,23 @@ cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::Step
   uint64_t want = (n + THREADS - 1) / THREADS;
   uint64_t cap = (uint64_t)g_num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
-  gray2::integrate_kernel<T, THREADS, MIN_BLOCKS><<<grid, THREADS, 0, st>>>(view_of<T>(s), n, p, queue, steps);
+  auto v = view_of<T>(s);
+  if (p.mode == 1) {
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+  } else {
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+  }
   return cudaGetLastError();
 }
 
 struct LaunchChoice { int threads, blocks; };
 
 // compiled variants; the first entry of each list is the default
-constexpr LaunchChoice kF64Variants[] = {{128, 3}, {128, 2}, {128, 4}, {64, 6}, {256, 1}, {64, 8}};
-constexpr LaunchChoice kF32Variants[] = {{128, 6}, {128, 4}, {128, 8}, {256, 3}, {256, 2}, {64, 12}};
+constexpr int kNumVariants = 3;
+constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}};
+constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 6}, {128, 8}, {256, 3}};
 
 template <typename T>
 cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, uint64_t n,
@@ -104,11 +112,9 @@ cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, ui
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL>(s, n, p, q, steps, st);
   if constexpr (sizeof(T) == 8) {
-    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 2) GRAY2_VARIANT(128, 4)
-    GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(64, 8)
+    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6)
   } else {
-    GRAY2_VARIANT(128, 6) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(128, 8)
-    GRAY2_VARIANT(256, 3) GRAY2_VARIANT(256, 2) GRAY2_VARIANT(64, 12)
+    GRAY2_VARIANT(128, 6) GRAY2_VARIANT(128, 8) GRAY2_VARIANT(256, 3)
   }
 #undef GRAY2_VARIANT
   *found = false;
@@ -124,6 +130,10 @@ int integrate_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_st
   p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
   p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
   p.r_escape = (T)sc->r_escape;
+  {
+    const double big = sizeof(T) == 8 ? 1.7976931348623157e308 : 3.402823466e38;
+    p.r_escape_fin = (T)(sc->r_escape < big ? sc->r_escape : big);
+  }
   p.lambda_end = lambda_end;
   p.dir = (double)sc->dir;
   p.mode = sc->mode;
@@ -267,9 +277,9 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
 }
 
 /* Source-level count of ks_geodesic.cuh (FMA = 2, add/mul = 1, rsqrt/rcp = 1; negations and compares free):
- *   radius 16, rest of geometry 54, velocity part 63  ->  133 per right-hand side
- *   4 x 133 + RK4 combination 100 + step rule and lambda update 2 = 634 per step (both precisions). */
-int gray2_flops_per_step(int32_t prec) { (void)prec; return 634; }
+ *   radius 16, rest of geometry 24, velocity part 73  ->  113 per right-hand side
+ *   4 x 113 + RK4 combination 100 + step rule and lambda update 2 = 554 per step (both precisions). */
+int gray2_flops_per_step(int32_t prec) { (void)prec; return 554; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
@@ -289,7 +299,7 @@ int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per
   if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_set_launch: unknown precision");
   const LaunchChoice *list = prec == GRAY2_F64 ? kF64Variants : kF32Variants;
   bool ok = threads_per_block == 0 && blocks_per_sm == 0;
-  for (int i = 0; i < 6 && !ok; ++i) ok = list[i].threads == threads_per_block && list[i].blocks == blocks_per_sm;
+  for (int i = 0; i < kNumVariants && !ok; ++i) ok = list[i].threads == threads_per_block && list[i].blocks == blocks_per_sm;
   if (!ok) return fail(GRAY2_EINVAL, "gray2_set_launch: %d x %d is not a compiled variant", threads_per_block, blocks_per_sm);
   g_threads[prec] = threads_per_block;
   g_blocks_per_sm[prec] = blocks_per_sm;

@@ -27,6 +27,7 @@ template <typename T> struct StepParams {
   T eta_or_h;          // eta (mode 1) or h_fixed (mode 0), already multiplied by dir
   T r_capture;         // capture_factor * r_plus
   T r_escape;
+  T r_escape_fin;     // min(r_escape, largest finite value of T)
   double lambda_end;
   double dir;
   int32_t mode;
@@ -82,7 +83,14 @@ __global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ 
 }
 
 // ---- the fused integrator ------------------------------------------------------------------------
-template <typename T, int THREADS, int MIN_BLOCKS>
+// MODE: 0 fixed step, 1 radius-scaled step.  CLIP: false only when dir*lambda_end = +inf, i.e. the
+// lambda_end test can never fire and the last step never needs clipping.
+//
+// Loop structure.  The outer loop refills idle lanes from the global queue; the inner loop advances
+// every lane of the warp by one RK4 step per pass and leaves as soon as ANY lane's stopping test fires
+// (one vote per step).  In the hot path the stopping rule of gray2_step_control costs four compares:
+// the tests are ordered only in the (rare) slow path that classifies and stores a finished ray.
+template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long *queue,
                  unsigned long long *steps_out) {
@@ -91,8 +99,10 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
   const SpinConst<T> k = p.k;
 
   Ray<T> ray;
+  ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = T(0);
+  ray.z = T(3);                // idle lanes integrate a harmless dummy state (never stored)
   double lam = 0.0;
-  int32_t nst = 0;
+  int32_t nst = 0, nst0 = 0;
   uint64_t idx = 0;
   bool have = false;           // this lane holds an ACTIVE geodesic
   bool drained = false;        // warp-uniform: the queue has no more work
@@ -103,9 +113,10 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
     unsigned idle = __ballot_sync(0xffffffffu, !have);
     if (idle && !drained) {
       unsigned cnt = __popc(idle);
+      int leader = __ffs(idle) - 1;
       unsigned long long base = 0;
-      if (lane == (unsigned)(__ffs(idle) - 1)) base = atomicAdd(queue, (unsigned long long)cnt);
-      base = __shfl_sync(0xffffffffu, base, __ffs(idle) - 1);
+      if ((int)lane == leader) base = atomicAdd(queue, (unsigned long long)cnt);
+      base = __shfl_sync(0xffffffffu, base, leader);
       if (base + cnt >= n) drained = true;
       if (!have) {
         uint64_t mine = base + __popc(idle & lt_mask);
@@ -114,49 +125,48 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
           ray.t = s.q[0][idx]; ray.x = s.q[1][idx]; ray.y = s.q[2][idx]; ray.z = s.q[3][idx];
           ray.u0 = s.q[4][idx]; ray.u1 = s.q[5][idx]; ray.u2 = s.q[6][idx]; ray.u3 = s.q[7][idx];
           lam = s.lambda[idx];
-          nst = s.nsteps[idx];
+          nst = nst0 = s.nsteps[idx];
           have = true;
         }
       }
-      continue;   // newly loaded lanes may need another refill (non-ACTIVE entries); tests run next pass
+      continue;   // entries that were not ACTIVE leave the lane idle: ask again
     }
     if (idle == 0xffffffffu) break;   // nothing held and the queue is drained
 
-    if (have) {
-      // ---- stopping tests on the current state, in the order of gray2_step_control ------------
+    // ---- step all lanes until one of them has to stop ---------------------------------------------
+    for (;;) {
       Geometry<T> g;
       ks_geometry(k, ray.x, ray.y, ray.z, g);
-      T U = fma_(g.l1, ray.u1, fma_(g.l2, ray.u2, fma_(g.l3, ray.u3, ray.u0)));
-      int32_t st = GRAY2_ACTIVE;
-      bool stop = false;
-      if (!(fastmath<T>::finite(g.r) && fastmath<T>::finite(U) && fastmath<T>::finite(ray.t))) {
-        st = GRAY2_INVALID; stop = true;
-      } else if (g.r < p.r_capture) {
-        st = GRAY2_CAPTURED; stop = true;
-      } else if (g.r > p.r_escape) {
-        st = GRAY2_ESCAPED; stop = true;
-      } else if (nst >= p.max_steps) {
-        st = GRAY2_MAXSTEPS; stop = true;
-      } else if (p.clip && p.dir * (p.lambda_end - lam) <= 0.0) {
-        stop = true;           // stays ACTIVE: resumable
-      }
-      if (stop) {
-        s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
-        s.q[4][idx] = ray.u0; s.q[5][idx] = ray.u1; s.q[6][idx] = ray.u2; s.q[7][idx] = ray.u3;
-        s.lambda[idx] = lam; s.status[idx] = st; s.nsteps[idx] = nst;
-        have = false;
-      } else {
-        T h = (p.mode == 1) ? p.eta_or_h * g.r : p.eta_or_h;
-        double hd = (double)h;
-        if (p.clip) {
-          double rem = p.lambda_end - lam;
-          if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
+      T U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+      // NaN fails every compare; r_escape_fin = min(r_escape, largest finite) so that r = inf fails too
+      bool go = (g.r >= p.r_capture) && (g.r <= p.r_escape_fin) && fastmath<T>::finite(U) &&
+                fastmath<T>::finite(ray.t) && (nst < p.max_steps);
+      if (CLIP) go = go && (p.dir * (p.lambda_end - lam) > 0.0);
+      if (__any_sync(0xffffffffu, have && !go)) {
+        if (have && !go) {
+          // classify in the order of gray2_step_control and store the state where the test fired
+          int32_t st = GRAY2_ACTIVE;    // lambda_end reached: stays ACTIVE (resumable)
+          if (!(fastmath<T>::finite(g.r) && fastmath<T>::finite(U) && fastmath<T>::finite(ray.t))) st = GRAY2_INVALID;
+          else if (g.r < p.r_capture) st = GRAY2_CAPTURED;
+          else if (g.r > p.r_escape) st = GRAY2_ESCAPED;
+          else if (nst >= p.max_steps) st = GRAY2_MAXSTEPS;
+          s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
+          s.q[4][idx] = ray.u0; s.q[5][idx] = ray.u1; s.q[6][idx] = ray.u2; s.q[7][idx] = ray.u3;
+          s.lambda[idx] = lam; s.status[idx] = st; s.nsteps[idx] = nst;
+          my_steps += (unsigned long long)(nst - nst0);
+          have = false;
         }
-        rk4_step(k, ray, g, h);
-        lam += hd;
-        nst += 1;
-        my_steps += 1;
+        break;
       }
+      T h = (MODE == 1) ? p.eta_or_h * g.r : p.eta_or_h;
+      double hd = (double)h;
+      if (CLIP) {
+        double rem = p.lambda_end - lam;
+        if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
+      }
+      rk4_step(k, ray, g, h);
+      lam += hd;
+      nst += 1;
     }
   }
 
@@ -200,7 +210,7 @@ __global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos
   Geometry<T> g;
   ks_geometry(k, pos[i], pos[n + i], pos[2 * n + i], g);
   T a0, a1, a2, a3;
-  ks_accel(g, u[i], u[n + i], u[2 * n + i], u[3 * n + i], a0, a1, a2, a3);
+  ks_accel(k, g, pos[i], pos[n + i], u[i], u[n + i], u[2 * n + i], u[3 * n + i], a0, a1, a2, a3);
   out[i] = a0; out[n + i] = a1; out[2 * n + i] = a2; out[3 * n + i] = a3;
 }
 

@@ -80,13 +80,19 @@ template <typename T> struct SpinConst {
 };
 
 // Position-only part of the right-hand side (shared by the stopping test, the step rule and stage 1).
+//
+// Final regrouping: with n = (x, y, zeta), zeta = z P / r^2, one has
+// grad r = (f/2) n and grad f = alpha n - beta e_z; the unit vector l and the vector A enter the spatial
+// acceleration only through  -c_A A_i - l_i xddot^0 , and both are combinations of (x, y) and
+// (r x + a y, r y - a x) / P, so that
+//   xddot^1 = kappa x + mu y - c_B u2 ,  xddot^2 = kappa y - mu x + c_B u1 ,
+//   xddot^3 = c_n zeta + l3 (c_A / r - xddot^0) - (U^2/2) beta
+// with scalars kappa, mu, c_n, c_A, c_B built from the dot products below: l1, l2, A1, A2 and curl l are
+// never formed.
 template <typename T> struct Geometry {
-  T r, rinv, Pinv, f, l1, l2, l3;
-  T rx, ry, rz;     // grad r
-  T fx, fy, fz;     // grad f
-  T lf;             // l . grad f
-  T w1, w2, w3;     // curl l
-  T A1, A2, A3, rP; // pieces of the symmetric part
+  T r, rinv, Pinv, hf, f, l3, zeta;
+  T alpha, beta, lf;        // grad f = alpha n - beta e_z ;  lf = l . grad f
+  T tr, trP, rP, taP;       // 2r, 2r/P, r/P, 2a/P
 };
 
 template <typename T>
@@ -109,53 +115,61 @@ __device__ __forceinline__ void ks_geometry(const SpinConst<T> &k, T x, T y, T z
   T P = r2 + k.a2;
   T Pinv = fastmath<T>::rcp(P);
   g.Pinv = Pinv;
-  T hf = r * Dinv;                 // f / 2
+  T hf = r * Dinv;                 // f / 2 = r / Sigma
   T f = hf + hf;
+  g.hf = hf;
   g.f = f;
-  g.l1 = fma_(r, x, k.a * y) * Pinv;
-  g.l2 = fma_(r, y, -k.a * x) * Pinv;
   g.l3 = z * rinv;
   T rinv2 = rinv * rinv;
-  g.rx = hf * x;
-  g.ry = hf * y;
-  g.rz = hf * (z * (P * rinv2));
+  g.zeta = z * (P * rinv2);
   T c1 = fma_(T(3), rinv, -(f + f));
   T c2 = k.two_a2 * z * (Dinv * rinv2);
-  T c1f = c1 * f;
-  g.fx = c1f * g.rx;
-  g.fy = c1f * g.ry;
-  g.fz = fma_(c1f, g.rz, -c2 * f);
+  g.alpha = (f * c1) * hf;
+  g.beta = c2 * f;
   g.lf = f * fma_(-c2, g.l3, c1);
-  T tr = r + r;
-  g.A1 = fma_(-tr, g.l1, x) * Pinv;
-  g.A2 = fma_(-tr, g.l2, y) * Pinv;
-  g.A3 = -g.l3 * rinv;
+  g.tr = r + r;
+  g.trP = g.tr * Pinv;
   g.rP = r * Pinv;
-  g.w1 = fma_(g.ry, g.A3, -g.rz * g.A2);
-  g.w2 = fma_(g.rz, g.A1, -g.rx * g.A3);
-  g.w3 = fma_(g.rx, g.A2, fma_(-g.ry, g.A1, -k.two_a * Pinv));
+  g.taP = k.two_a * Pinv;
 }
 
-// Velocity-dependent part: xddot^mu from the geometry and u (eq. 13-14).
+// Velocity-dependent part: xddot^mu from the geometry, the position and u (eq. 13-14).
 template <typename T>
-__device__ __forceinline__ void ks_accel(const Geometry<T> &g, T u0, T u1, T u2, T u3,
-                                         T &a0, T &a1, T &a2, T &a3) {
-  T U = fma_(g.l1, u1, fma_(g.l2, u2, fma_(g.l3, u3, u0)));
-  T ur = fma_(u1, g.rx, fma_(u2, g.ry, u3 * g.rz));
-  T Au = fma_(u1, g.A1, fma_(u2, g.A2, u3 * g.A3));
+__device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T> &g, T x, T y,
+                                         T u0, T u1, T u2, T u3, T &a0, T &a1, T &a2, T &a3) {
+  T xu = fma_(x, u1, y * u2);
+  T yu = fma_(y, u1, -x * u2);
+  T lu = g.Pinv * fma_(g.r, xu, k.a * yu);        // l1 u1 + l2 u2
+  T zu = g.l3 * u3;
+  T U = (u0 + lu) + zu;                            // l_alpha u^alpha
+  T Au = fma_(g.Pinv, fma_(-g.tr, lu, xu), -zu * g.rinv);
+  T unv = fma_(g.zeta, u3, xu);                    // n . u
+  T ur = g.hf * unv;                               // u . grad r
   T s12 = fma_(u1, u1, u2 * u2);
   T q = fma_(ur, Au, fma_(g.rP, s12, (u3 * u3) * g.rinv));
-  T uf = fma_(u1, g.fx, fma_(u2, g.fy, u3 * g.fz));
+  T uf = fma_(g.alpha, unv, -g.beta * u3);         // u . grad f
   T hU2 = T(0.5) * (U * U);
   T fU = g.f * U;
-  T G = fma_(U, uf, g.f * q);
-  a0 = fma_(g.f * hU2, g.lf, G);               // G - F,  F = -f (U^2/2) (l.grad f)
-  T c1 = fma_(u2, g.w3, -u3 * g.w2);           // u x omega
-  T c2 = fma_(u3, g.w1, -u1 * g.w3);
-  T c3 = fma_(u1, g.w2, -u2 * g.w1);
-  a1 = fma_(hU2, g.fx, fma_(fU, c1, -g.l1 * a0));
-  a2 = fma_(hU2, g.fy, fma_(fU, c2, -g.l2 * a0));
-  a3 = fma_(hU2, g.fz, fma_(fU, c3, -g.l3 * a0));
+  a0 = fma_(g.f * hU2, g.lf, fma_(U, uf, g.f * q));
+  T cn = fma_(fU * g.hf, Au, hU2 * g.alpha);
+  T cA = fU * ur;
+  T cB = fU * g.taP;
+  T e1 = -cA * g.Pinv;
+  T e2 = g.Pinv * fma_(cA, g.trP, -a0);
+  T kap = fma_(e2, g.r, cn + e1);
+  T mu = e2 * k.a;
+  a1 = fma_(kap, x, fma_(mu, y, -cB * u2));
+  a2 = fma_(kap, y, fma_(-mu, x, cB * u1));
+  a3 = fma_(cn, g.zeta, fma_(g.l3, fma_(cA, g.rinv, -a0), -hU2 * g.beta));
+}
+
+// l_alpha u^alpha alone (finite-ness test of the velocity at the top of a step).
+template <typename T>
+__device__ __forceinline__ T ks_U(const SpinConst<T> &k, const Geometry<T> &g, T x, T y, T u0, T u1, T u2, T u3) {
+  T xu = fma_(x, u1, y * u2);
+  T yu = fma_(y, u1, -x * u2);
+  T lu = g.Pinv * fma_(g.r, xu, k.a * yu);
+  return (u0 + lu) + g.l3 * u3;
 }
 
 // One geodesic's 8 variables.
@@ -174,28 +188,28 @@ __device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const
   T St, Sx, Sy, Sz, S0, S1, S2, S3;      // k1 + 2 k2 + 2 k3 (+ k4)
   Geometry<T> g;
   // stage 1
-  ks_accel(g1, s.u0, s.u1, s.u2, s.u3, b0, b1, b2, b3);
+  ks_accel(k, g1, s.x, s.y, s.u0, s.u1, s.u2, s.u3, b0, b1, b2, b3);
   St = s.u0; Sx = s.u1; Sy = s.u2; Sz = s.u3;
   S0 = b0; S1 = b1; S2 = b2; S3 = b3;
   px = fma_(hh, s.u1, s.x); py = fma_(hh, s.u2, s.y); pz = fma_(hh, s.u3, s.z);
   v0 = fma_(hh, b0, s.u0); v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
   // stage 2
   ks_geometry(k, px, py, pz, g);
-  ks_accel(g, v0, v1, v2, v3, b0, b1, b2, b3);
+  ks_accel(k, g, px, py, v0, v1, v2, v3, b0, b1, b2, b3);
   St = fma_(T(2), v0, St); Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
   S0 = fma_(T(2), b0, S0); S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
   px = fma_(hh, v1, s.x); py = fma_(hh, v2, s.y); pz = fma_(hh, v3, s.z);
   v0 = fma_(hh, b0, s.u0); v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
   // stage 3
   ks_geometry(k, px, py, pz, g);
-  ks_accel(g, v0, v1, v2, v3, b0, b1, b2, b3);
+  ks_accel(k, g, px, py, v0, v1, v2, v3, b0, b1, b2, b3);
   St = fma_(T(2), v0, St); Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
   S0 = fma_(T(2), b0, S0); S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
   px = fma_(h, v1, s.x); py = fma_(h, v2, s.y); pz = fma_(h, v3, s.z);
   v0 = fma_(h, b0, s.u0); v1 = fma_(h, b1, s.u1); v2 = fma_(h, b2, s.u2); v3 = fma_(h, b3, s.u3);
   // stage 4
   ks_geometry(k, px, py, pz, g);
-  ks_accel(g, v0, v1, v2, v3, b0, b1, b2, b3);
+  ks_accel(k, g, px, py, v0, v1, v2, v3, b0, b1, b2, b3);
   s.t = fma_(h6, St + v0, s.t);
   s.x = fma_(h6, Sx + v1, s.x);
   s.y = fma_(h6, Sy + v2, s.y);

@@ -105,7 +105,7 @@ def test_results_do_not_depend_on_launch_shape_or_run():
     cfg = inputs.CFG3_NULL.scaled(150, 90)
     ref = None
     try:
-        for shape in [(0, 0), (128, 2), (64, 6), (256, 1), (0, 0)]:
+        for shape in [(0, 0), (128, 4), (64, 6), (0, 0)]:
             gray2.set_launch(gray2.F64, *shape)
             _, g, stats = run_gpu_image(cfg)
             cur = (g.q.clone(), g.nsteps.clone(), g.status.clone(), g.lam.clone(), stats)
