@@ -260,16 +260,19 @@ def run_gpu(args):
     e2e_steps = sum(e2e_step() for _ in range(e2e_n))
     t_e2e = time.perf_counter() - t0
 
-    # ---- FMA-only probe of the pipe at the clocks of the moment (context for the nominal peak)
+    # ---- FMA-only probes of the pipe at the clocks of the moment (context for the nominal peak)
     scratch = torch.zeros(8, dtype=torch.float64 if prec == gray2.F64 else torch.float32, device="cuda")
     iters = 20000 if prec == gray2.F64 else 40000
-    gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    probe_flops = gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch)
-    e1.record(stream)
-    e1.synchronize()
-    fma_probe_tflops = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
+    probe = {}
+    for name, regs in (("imm", False), ("regs", True)):
+        gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch, register_operands=regs)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        probe_flops = gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch, register_operands=regs)
+        e1.record(stream)
+        e1.synchronize()
+        probe[name] = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
+    fma_probe_tflops = probe["imm"]
 
     # ---- reduce over ranks: time = max, work = sum
     from paper_1706_07062_b200 import multi
@@ -297,7 +300,8 @@ def run_gpu(args):
                          "traffic": None, "flops_per_rk4_step": flops_per_step,
                          "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,
                          "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (n_sms, FP_LANES[args.dtype], sm_max_mhz),
-                         "fma_probe_tflops": fma_probe_tflops, "frac_of_fma_probe": achieved / fma_probe_tflops},
+                         "fma_probe_tflops": fma_probe_tflops, "frac_of_fma_probe": achieved / fma_probe_tflops,
+                         "fma_probe_register_operands_tflops": probe["regs"]},
         }
         if not args.no_cpu_baseline and world == 1:
             v, s_per, cores, sub = time_oracle(cfg, args.oracle_side, 1, 0)

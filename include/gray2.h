@@ -125,8 +125,11 @@ int gray2_flops_per_step(int32_t prec);
 int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream);
 
 /* Diagnostic entry: FMA-only probe kernel (8 independent chains per thread) for measuring the attainable
- * FMA rate of the FP64 / FP32 pipe.  scratch: DEVICE pointer, >= 1 element.  Flops = 16*iters*blocks*threads. */
-int gray2_fma_probe(int32_t prec, int32_t blocks, int32_t threads, int32_t iters, void *scratch, void *cuda_stream);
+ * FMA rate of the FP64 / FP32 pipe.  register_operands = 0: multiplier and addend are immediates (best
+ * case of the pipe); 1: three per-thread register operands (what real code issues; bounded by register-file
+ * read bandwidth).  scratch: DEVICE pointer, >= 1 element.  Flops = 16*iters*blocks*threads. */
+int gray2_fma_probe(int32_t prec, int32_t register_operands, int32_t blocks, int32_t threads, int32_t iters,
+                    void *scratch, void *cuda_stream);
 
 const char *gray2_last_error(void);   /* thread-local text of the last error of the calling thread */
 const char *gray2_version(void);

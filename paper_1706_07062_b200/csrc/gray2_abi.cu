@@ -100,9 +100,9 @@ cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::Step
 struct LaunchChoice { int threads, blocks; };
 
 // compiled variants; the first entry of each list is the default
-constexpr int kNumVariants = 3;
-constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}};
-constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 6}, {128, 8}, {256, 3}};
+constexpr int kNumVariants = 5;
+constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}, {128, 2}, {256, 1}};
+constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 8}, {128, 6}, {256, 3}, {128, 4}, {128, 3}};
 
 template <typename T>
 cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, uint64_t n,
@@ -112,9 +112,9 @@ cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, ui
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL>(s, n, p, q, steps, st);
   if constexpr (sizeof(T) == 8) {
-    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6)
+    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(128, 2) GRAY2_VARIANT(256, 1)
   } else {
-    GRAY2_VARIANT(128, 6) GRAY2_VARIANT(128, 8) GRAY2_VARIANT(256, 3)
+    GRAY2_VARIANT(128, 6) GRAY2_VARIANT(128, 8) GRAY2_VARIANT(256, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(128, 3)
   }
 #undef GRAY2_VARIANT
   *found = false;
@@ -283,14 +283,20 @@ int gray2_flops_per_step(int32_t prec) { (void)prec; return 554; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
+ * register_operands = 0: multiplier and addend are immediates; 1: three per-thread register operands.
  * scratch: DEVICE pointer to at least one element of the precision's type.  Flops = 16*iters*blocks*threads. */
-int gray2_fma_probe(int32_t prec, int32_t blocks, int32_t threads, int32_t iters, void *scratch, void *cuda_stream) {
+int gray2_fma_probe(int32_t prec, int32_t register_operands, int32_t blocks, int32_t threads, int32_t iters,
+                    void *scratch, void *cuda_stream) {
   if (!scratch || blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0)
     return fail(GRAY2_EINVAL, "gray2_fma_probe: bad argument");
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  if (prec == GRAY2_F64) gray2::fma_probe_kernel<double><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
-  else if (prec == GRAY2_F32) gray2::fma_probe_kernel<float><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
-  else return fail(GRAY2_EINVAL, "gray2_fma_probe: unknown precision");
+  if (prec == GRAY2_F64) {
+    if (register_operands) gray2::fma_probe_kernel<double, true><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
+    else gray2::fma_probe_kernel<double, false><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
+  } else if (prec == GRAY2_F32) {
+    if (register_operands) gray2::fma_probe_kernel<float, true><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+    else gray2::fma_probe_kernel<float, false><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+  } else return fail(GRAY2_EINVAL, "gray2_fma_probe: unknown precision");
   CUDA_TRY(cudaGetLastError());
   return GRAY2_OK;
 }

@@ -216,12 +216,16 @@ __global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos
 
 // Diagnostic: FMA-only probe of the FP64 / FP32 pipe (8 independent chains per thread, registers only).
 // Each thread executes 8 * iters FMAs; the launch's flop count is 2 * 8 * iters * threads.
-template <typename T>
+// REGS = false: multiplier and addend are immediates (the pipe's best case);
+// REGS = true : all three operands are registers that differ per thread, as in real code, which on
+//               B200 is limited by register-file read bandwidth rather than by the pipe.
+template <typename T, bool REGS>
 __global__ void fma_probe_kernel(int iters, T seed, T *__restrict__ out) {
   T a0 = seed + T(threadIdx.x), a1 = a0 + T(1), a2 = a0 + T(2), a3 = a0 + T(3);
   T a4 = a0 + T(4), a5 = a0 + T(5), a6 = a0 + T(6), a7 = a0 + T(7);
-  const T m = T(0.999999), c = T(1e-6);
-#pragma unroll 4
+  const T m = REGS ? T(0.999999) + T(threadIdx.x) * T(1e-9) : T(0.999999);
+  const T c = REGS ? T(1e-6) + T(threadIdx.x) * T(1e-9) : T(1e-6);
+#pragma unroll 8
   for (int i = 0; i < iters; ++i) {
     a0 = fma_(a0, m, c); a1 = fma_(a1, m, c); a2 = fma_(a2, m, c); a3 = fma_(a3, m, c);
     a4 = fma_(a4, m, c); a5 = fma_(a5, m, c); a6 = fma_(a6, m, c); a7 = fma_(a7, m, c);

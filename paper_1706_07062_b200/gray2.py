@@ -70,7 +70,7 @@ def load_library():
     lib.gray2_invariants.argtypes = [p, u64, p, p, p, p, p]
     lib.gray2_rhs.argtypes = [i32, d, u64, p, p, p, p]
     lib.gray2_set_launch.argtypes = [i32, i32, i32]
-    lib.gray2_fma_probe.argtypes = [i32, i32, i32, i32, p, p]
+    lib.gray2_fma_probe.argtypes = [i32, i32, i32, i32, i32, p, p]
     lib.gray2_fma_probe.restype = C.c_int
     lib.gray2_flops_per_step.argtypes = [i32]
     for name in ("gray2_init_null", "gray2_init_timelike", "gray2_integrate", "gray2_invariants", "gray2_rhs",
@@ -203,9 +203,10 @@ def rhs(prec, a, pos: torch.Tensor, u: torch.Tensor, stream=None) -> torch.Tenso
     return out
 
 
-def fma_probe(prec, blocks, threads, iters, scratch: torch.Tensor, stream=None):
+def fma_probe(prec, blocks, threads, iters, scratch: torch.Tensor, register_operands=False, stream=None):
     """Diagnostic: enqueue the FMA-only probe kernel; flops = 16 * iters * blocks * threads."""
-    _check(load_library().gray2_fma_probe(prec, blocks, threads, iters, C.c_void_p(scratch.data_ptr()),
+    _check(load_library().gray2_fma_probe(prec, int(register_operands), blocks, threads, iters,
+                                          C.c_void_p(scratch.data_ptr()),
                                           _stream_ptr(stream)))
     return 16 * iters * blocks * threads
 
