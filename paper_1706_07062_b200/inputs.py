@@ -177,6 +177,8 @@ def solve_orbit_constants(a, p, e, cosi, iters=60):
         sE = np.clip(sE, -0.05, 0.05)
         sL = np.clip(sL, -1.0, 1.0)
         E, L = E - sE, L - sL
+        if _ >= 4 and float(np.max(np.abs(sE))) < 1e-15 and float(np.max(np.abs(sL) / np.maximum(L, 1.0))) < 1e-15:
+            break
     f1, f2 = F(E, L)
     scale = rp ** 4
     ok &= (np.abs(f1) < 1e-9 * scale) & (np.abs(f2) < 1e-9 * scale / rp) & (L > 0) & np.isfinite(E)

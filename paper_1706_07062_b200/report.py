@@ -1,0 +1,164 @@
+"""Run the five BASELINE.json configs on the GPU and print one JSON report (GPU-only statistics).
+
+    python -m paper_1706_07062_b200.report [--configs 1,2,3,4,5] [--cfg4-steps 100000] [--cfg4-n 1048576]
+
+What each config asks to be reported (BASELINE.json "configs"):
+  cfg1  Schwarzschild 64x64 image + 16 time-like orbits: status counts, step counts, invariant drift
+  cfg2  Kerr a=0.99 512x512: status counts; the critical band is reported as the rays with unusually long paths
+  cfg3  Kerr a=0.9375 1024x1024 in FP64 and FP32: FP32-vs-FP64 error on final (r, theta, phi) of escaped
+        rays and on the capture mask
+  cfg4  1,048,576 bound particles, fixed step 0.5, 100,000 steps: drift of E, L_z, Q and u.u
+  cfg5  Kerr a=0.5 4096x4096 in FP32 and FP64: throughput under divergence in path length
+The oracle comparisons live in tests/ (this module never touches the oracle).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import time
+
+import torch
+
+from . import gray2, inputs
+
+INF = float("inf")
+
+
+def _timed(fn):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    out = fn()
+    e1.record()
+    e1.synchronize()
+    return out, e0.elapsed_time(e1) * 1e-3
+
+
+def run_image(cfg, prec):
+    sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
+                            capture_factor=cfg.capture_factor)
+    st = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec)
+    inv0 = gray2.invariants(st)
+    stats = gray2.new_stats()
+    gray2.integrate(st, INF, sc, stats=stats)          # warm-up launch on a copy would double memory: time a rerun
+    torch.cuda.synchronize()
+    st2 = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st)
+    _, dt = _timed(lambda: gray2.integrate(st2, INF, sc, stats=stats))
+    inv1 = gray2.invariants(st2)
+    sd = gray2.stats_dict(stats)
+    ns = st2.nsteps
+    esc = st2.status == gray2.ESCAPED
+    rep = dict(sd, rays=cfg.n, seconds=dt, steps_per_s=sd["steps"] / dt,
+               nsteps_min=int(ns.min()), nsteps_mean=float(ns.float().mean()), nsteps_max=int(ns.max()),
+               captured_fraction=sd["n_captured"] / cfg.n,
+               long_path_rays=int((ns > 1.5 * ns.float().mean()).sum()),
+               max_abs_norm_escaped=float(inv1[3][esc].abs().max()),
+               max_drift_E_escaped=float((inv1[0] - inv0[0])[esc].abs().max()),
+               max_drift_Lz_escaped=float((inv1[1] - inv0[1])[esc].abs().max()),
+               max_drift_Q_escaped=float((inv1[2] - inv0[2])[esc].abs().max()))
+    return st2, rep
+
+
+def spherical(q, a_eff):
+    """KS r, theta, phi of positions q[1:4] (torch, double): x + i y = (r + i a) sin(theta) e^{i phi}."""
+    x, y, z = q[1].double(), q[2].double(), q[3].double()
+    w = x * x + y * y + z * z - a_eff * a_eff
+    r = torch.sqrt(0.5 * (w + torch.sqrt(w * w + 4 * a_eff * a_eff * z * z)))
+    th = torch.acos(torch.clamp(z / r, -1.0, 1.0))
+    ph = torch.atan2(y, x) - torch.atan2(torch.full_like(r, a_eff), r)
+    return r, th, ph
+
+
+def report_cfg3():
+    cfg = inputs.CFG3_NULL
+    s64, r64 = run_image(cfg, gray2.F64)
+    s32, r32 = run_image(cfg, gray2.F32)
+    both_esc = (s64.status == gray2.ESCAPED) & (s32.status == gray2.ESCAPED)
+    same = both_esc & (s64.nsteps == s32.nsteps)
+    ra, ta, pa = spherical(s64.q, s64.a_eff)
+    rb, tb, pb = spherical(s32.q, s32.a_eff)
+    dphi = torch.remainder(pb - pa + math.pi, 2 * math.pi) - math.pi
+    err = {"r_rel": ((rb - ra).abs() / ra)[same], "theta": (tb - ta).abs()[same], "phi": dphi.abs()[same]}
+    qs = torch.tensor([0.5, 0.9, 0.99, 0.999, 1.0], dtype=torch.float64, device="cuda")
+
+    def quant(v):
+        v = v.double()
+        k = (qs * (v.numel() - 1)).long()
+        return [float(x) for x in torch.sort(v).values[k]]
+
+    # direction of the spatial velocity at the stopping state: insensitive to a +-1 step difference
+    va = s64.q[5:8].double()
+    vb = s32.q[5:8].double()
+    cosang = (va * vb).sum(0) / (va.norm(dim=0) * vb.norm(dim=0))
+    ang = torch.acos(torch.clamp(cosang, -1.0, 1.0))[both_esc]
+    mask_diff = int(((s64.status == gray2.CAPTURED) != (s32.status == gray2.CAPTURED)).sum())
+    return {"f64": r64, "f32": r32,
+            "fp32_vs_fp64": {"escaped_in_both": int(both_esc.sum()), "equal_step_count_fraction": float(same.sum()) / max(int(both_esc.sum()), 1),
+                             "quantiles": [0.5, 0.9, 0.99, 0.999, 1.0],
+                             "final_r_relative": quant(err["r_rel"]), "final_theta_rad": quant(err["theta"]),
+                             "final_phi_rad": quant(err["phi"]), "velocity_direction_rad_all_escaped": quant(ang),
+                             "capture_mask_disagreements": mask_diff, "rays": cfg.n}}
+
+
+def report_cfg1():
+    _, img = run_image(inputs.CFG1_NULL, gray2.F64)
+    xu8, r0 = inputs.cfg1_orbits()
+    st = gray2.init_timelike(0.0, xu8)
+    inv0 = gray2.invariants(st)
+    stats = gray2.new_stats()
+    gray2.integrate(st, INF, gray2.step_control(mode=0, h_fixed=0.5, max_steps=5000), stats=stats)
+    inv1 = gray2.invariants(st)
+    r = spherical(st.q, 0.0)[0].cpu()
+    orb = dict(gray2.stats_dict(stats), max_abs_r_minus_r0=float((r - torch.tensor(r0)).abs().max()),
+               max_drift=[float((b - a_).abs().max()) for a_, b in zip(inv0, inv1)])
+    return {"image": img, "orbits": orb}
+
+
+def report_cfg4(n, nsteps):
+    t0 = time.time()
+    xu8, meta = inputs.cfg4_ensemble(n)
+    gen_s = time.time() - t0
+    st = gray2.init_timelike(0.7, xu8)
+    inv0 = gray2.invariants(st)
+    stats = gray2.new_stats()
+    sc = gray2.step_control(mode=0, h_fixed=0.5, max_steps=nsteps)
+    _, dt = _timed(lambda: gray2.integrate(st, INF, sc, stats=stats))
+    inv1 = gray2.invariants(st)
+    sd = gray2.stats_dict(stats)
+    names = ("E", "Lz", "Q", "norm")
+    drift = {}
+    alive = st.status == gray2.MAXSTEPS     # a few marginal orbits plunge at this step size; they end inside 1.01 r_plus
+    for nm, a_, b in zip(names, inv0, inv1):
+        d = (b - a_)[alive]
+        rel = d / torch.clamp(a_[alive].abs(), min=1.0)
+        drift[nm] = {"max_abs": float(d.abs().max()), "rms": float(d.pow(2).mean().sqrt()),
+                     "max_rel_to_max(1,|value|)": float(rel.abs().max())}
+    return dict(sd, particles=n, steps_per_particle=nsteps, seconds=dt, steps_per_s=sd["steps"] / dt,
+                generator_seconds=gen_s, acceptance=meta["acceptance"], drift_of_particles_still_orbiting=drift)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", default="1,2,3,4,5")
+    ap.add_argument("--cfg4-steps", type=int, default=100000)
+    ap.add_argument("--cfg4-n", type=int, default=1 << 20)
+    args = ap.parse_args()
+    want = set(args.configs.split(","))
+    out = {"device": torch.cuda.get_device_name(0), "library": gray2.version()}
+    if "1" in want:
+        out["cfg1"] = report_cfg1()
+    if "2" in want:
+        out["cfg2"] = {"f64": run_image(inputs.CFG2_NULL, gray2.F64)[1]}
+    if "3" in want:
+        out["cfg3"] = report_cfg3()
+    if "4" in want:
+        out["cfg4"] = report_cfg4(args.cfg4_n, args.cfg4_steps)
+    if "5" in want:
+        out["cfg5"] = {"f32": run_image(inputs.CFG5_NULL, gray2.F32)[1]}
+        torch.cuda.empty_cache()
+        out["cfg5"]["f64"] = run_image(inputs.CFG5_NULL, gray2.F64)[1]
+    print(json.dumps(out, indent=1))
+
+
+if __name__ == "__main__":
+    main()

@@ -190,3 +190,80 @@ def test_cfg4_ensemble_sample_parity_and_drift():
     for k in range(4):
         scale = scales[k]
         assert np.max(np.abs((gi1[k] - gi0[k]) - (oi1[k] - oi0[k])) / scale) < 1e-12
+
+
+def test_cfg4_full_size_sampled_parity():
+    """BASELINE.json configs[3] at full size (1,048,576 particles x 100,000 fixed steps) in the launch
+    configuration bench.py uses; 64 sampled particles against the oracle."""
+    n, nsteps = 1 << 20, 100000
+    xu8, meta = inputs.cfg4_ensemble(n)
+    gsc, osc = sc_pair(mode=0, h_fixed=0.5, max_steps=nsteps)
+    g = gray2.init_timelike(0.7, xu8)
+    gi0 = [t.cpu().numpy() for t in gray2.invariants(g)]
+    stats = gray2.new_stats()
+    gray2.integrate(g, INF, gsc, stats=stats)
+    sd = gray2.stats_dict(stats)
+    assert sd["n_invalid"] == 0 and sd["n_active"] == 0 and sd["n_escaped"] == 0
+    assert sd["n_maxsteps"] + sd["n_captured"] == n and sd["n_captured"] < 100     # marginal orbits may plunge at h = 0.5
+    assert sd["steps"] == int(g.nsteps.sum(dtype=torch.int64).item())
+    idx = np.arange(0, n, n // 64)[:64]
+    o = oracle.init_timelike(0.7, xu8[idx])
+    oi0 = oracle.invariants(o)
+    oracle.integrate(o, INF, osc)
+    tidx = torch.tensor(idx, device="cuda")
+    assert np.array_equal(g.nsteps[tidx].cpu().numpy(), o.nsteps) and np.array_equal(g.status[tidx].cpu().numpy(), o.status)
+    err = state_rel_error(g.q[:, tidx].cpu().numpy(), o.q, 0.7)
+    assert err.max() < TOL_STATE_F64, err.max()
+    gi1 = [t.cpu().numpy() for t in gray2.invariants(g)]
+    oi1 = oracle.invariants(o)
+    from gpu_helpers import invariant_term_scales
+    scales = invariant_term_scales(o.q)
+    for k in range(4):
+        assert np.max(np.abs((gi1[k] - gi0[k])[idx] - (oi1[k] - oi0[k])) / scales[k]) < 1e-12
+    # drift stays at the RK4 truncation level over 1e5 steps
+    alive = g.status.cpu().numpy() == gray2.MAXSTEPS      # the few plunging particles end inside the horizon region
+    dE, dn = (gi1[0] - gi0[0])[alive], (gi1[3] - gi0[3])[alive]
+    assert np.abs(dE).max() < 1e-2 and np.abs(dn).max() < 1e-2              # worst: deep-periapsis orbits at h = 0.5
+    assert np.sqrt(np.mean(dE ** 2)) < 1e-4 and np.sqrt(np.mean(dn ** 2)) < 1e-4
+
+
+@pytest.mark.parametrize("prec", [gray2.F64, gray2.F32], ids=["f64", "f32"])
+def test_cfg5_full_size_sampled_parity(prec):
+    """BASELINE.json configs[4]: 4096 x 4096 rays (16.8 M), heavy divergence in path length."""
+    cfg = inputs.CFG5_NULL
+    gsc, osc = image_sc(cfg)
+    g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec)
+    stats = gray2.new_stats()
+    gray2.integrate(g, INF, gsc, stats=stats)
+    sd = gray2.stats_dict(stats)
+    assert sd["n_active"] == 0 and sd["n_invalid"] == 0 and sd["n_maxsteps"] <= 4
+    assert sd["n_captured"] + sd["n_escaped"] + sd["n_maxsteps"] == cfg.n
+    assert sd["steps"] == int(g.nsteps.sum(dtype=torch.int64).item())
+    ca, cb = __import__("closed_forms").bardeen_curve(cfg.a, cfg.inclination)
+    order = np.argsort(ca)
+    area = 2.0 * np.trapezoid(cb[order], ca[order])
+    assert abs(sd["n_captured"] / cfg.n - area / (2 * cfg.fov) ** 2) < 1e-3
+    rng = np.random.default_rng(5)
+    idx = np.sort(rng.choice(cfg.n, 768, replace=False))
+    full0 = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    o0 = take(full0, idx)
+    del full0
+    o = o0.copy()
+    oracle.integrate(o, INF, osc)
+    tidx = torch.tensor(idx, device="cuda")
+    gq = g.q[:, tidx].double().cpu().numpy()
+    gs, gn = g.status[tidx].cpu().numpy(), g.nsteps[tidx].cpu().numpy()
+    xi, eta, _, _ = ih.ray_constants(o0)
+    alpha, beta = ih.pixel_grid(cfg)
+    a_inf, b_inf = ih.asymptotic_image_point(o0.a_eff, cfg.inclination, xi, eta, np.where(beta[idx] >= 0, 1.0, -1.0))
+    d = ih.band_distance(cfg.a, cfg.inclination, a_inf, b_inf)
+    if prec == gray2.F64:
+        outside = d > 1e-3
+        assert np.array_equal(gs[outside], o.status[outside]) and np.array_equal(gn[outside], o.nsteps[outside])
+        assert state_rel_error(gq[:, outside], o.q[:, outside], o.a_eff).max() < TOL_STATE_F64
+    else:
+        outside = d > 2e-2
+        assert np.array_equal(gs[outside], o.status[outside])
+        same = outside & (gn == o.nsteps)
+        err = state_rel_error(gq[1:][:, same], o.q[1:][:, same], o.a_eff)
+        assert same.sum() > 0.5 * outside.sum() and np.quantile(err, 0.9) < 1e-4
