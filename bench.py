@@ -169,6 +169,11 @@ def run_gpu(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:                       # in-tree build (a no-op when libgray2.so is up to date)
+        from paper_1706_07062_b200 import build as _build
+        _build.build()
+    if world > 1:
+        dist.barrier()
     gray2.load_library()
 
     cfg = workload_config(args.workload)

@@ -81,6 +81,10 @@ def lib():
         _lib.oracle_init_timelike.argtypes = [p, d, p, C.c_uint64, C.c_int32]
         _lib.oracle_integrate.argtypes = [p, C.c_uint64, d, p, p]
         _lib.oracle_invariants.argtypes = [p, C.c_uint64, p, p, p, p]
+        _lib.oracle_ks_coordtime_accel.argtypes = [d, p, p, p]
+        _lib.oracle_rk4_step_coordtime.argtypes = [d, p, d]
+        _lib.oracle_trajectory_coordtime.argtypes = [d, p, d, C.c_int64, C.c_int64, p]
+        _lib.oracle_integrate_coordtime.argtypes = [p, C.c_uint64, d, p, p]
         _lib.oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -174,6 +178,17 @@ def integrate(st: State, lambda_end, sc: _StepControl, n=None) -> dict:
     return {k: int(getattr(stats, k)) for k, _ in _Stats._fields_}
 
 
+def integrate_coordtime(st: State, t_end, sc: _StepControl, n=None) -> dict:
+    """Coordinate-time form (eq. 15): see oracle_integrate_coordtime in gray2_oracle.h."""
+    cs = st._c()
+    stats = _Stats()
+    rc = lib().oracle_integrate_coordtime(C.byref(cs), st.n if n is None else n, float(t_end),
+                                          C.byref(sc), C.byref(stats))
+    if rc:
+        raise ValueError("oracle_integrate_coordtime: invalid arguments")
+    return {k: int(getattr(stats, k)) for k, _ in _Stats._fields_}
+
+
 def invariants(st: State):
     """Returns E, Lz, Q, norm (each (n,) float64) of the RUN geodesic (see gray2.h sign rule)."""
     out = [np.empty(st.n, dtype=np.float64) for _ in range(4)]
@@ -253,6 +268,21 @@ def trajectory(a, y0, h, nsteps, stride=1):
     y0 = _vec(y0, 8)
     out = np.empty((nsteps // stride + 1, 8), dtype=np.float64)
     lib().oracle_trajectory(a, _ptr(y0), h, nsteps, stride, _ptr(out))
+    return out
+
+
+def ks_coordtime_accel(a, pos, v):
+    pos, v = _vec(pos, 3), _vec(v, 3)
+    out = np.empty(3, dtype=np.float64)
+    lib().oracle_ks_coordtime_accel(a, _ptr(pos), _ptr(v), _ptr(out))
+    return out
+
+
+def trajectory_coordtime(a, y0, h, nsteps, stride=1):
+    """y0 = (t,x,y,z,vx,vy,vz); rows of the result likewise."""
+    y0 = _vec(y0, 7)
+    out = np.empty((nsteps // stride + 1, 7), dtype=np.float64)
+    lib().oracle_trajectory_coordtime(a, _ptr(y0), h, nsteps, stride, _ptr(out))
     return out
 
 

@@ -377,6 +377,100 @@ int oracle_integrate(oracle_state *s, uint64_t n, double lambda_end,
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Coordinate-time integration (section 2.2).  v^mu = dx^mu/dt, v^0 = 1.
+ * PAPER.md:131 eq. (15), literally, with the full connection:
+ *   dv^i/dt = -Gamma^i_ab v^a v^b + Gamma^0_ab v^a v^b v^i
+ * Six variables (x^i, v^i); t advances by exactly h per step.  The 8-array state is reused:
+ * on entry v^i = u^i / u^t, on exit q[4] = 1 and q[5..7] = v^i (DESIGN R19).
+ * ---------------------------------------------------------------------------------------- */
+void oracle_ks_coordtime_accel(double a, const double pos[3], const double v[3], double dv[3])
+{
+  double Gam[64], u[4] = { 1.0, v[0], v[1], v[2] }, acc[4];
+  oracle_ks_christoffel(a, pos, Gam);
+  accel_from(Gam, u, acc);               /* acc^mu = -Gamma^mu_ab v^a v^b */
+  for (int i = 0; i < 3; ++i) dv[i] = acc[1 + i] - acc[0] * v[i];
+}
+
+/* y = (x,y,z,vx,vy,vz); classic RK4 in t. */
+static void ct_deriv(double a, const double y[6], double dy[6])
+{
+  for (int i = 0; i < 3; ++i) dy[i] = y[3 + i];
+  oracle_ks_coordtime_accel(a, &y[0], &y[3], &dy[3]);
+}
+
+void oracle_rk4_step_coordtime(double a, double y[6], double h)
+{
+  double k1[6], k2[6], k3[6], k4[6], w[6];
+  ct_deriv(a, y, k1);
+  for (int i = 0; i < 6; ++i) w[i] = y[i] + 0.5 * h * k1[i];
+  ct_deriv(a, w, k2);
+  for (int i = 0; i < 6; ++i) w[i] = y[i] + 0.5 * h * k2[i];
+  ct_deriv(a, w, k3);
+  for (int i = 0; i < 6; ++i) w[i] = y[i] + h * k3[i];
+  ct_deriv(a, w, k4);
+  for (int i = 0; i < 6; ++i) y[i] = y[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+}
+
+/* fixed-step trajectory in t: out rows are (t,x,y,z,vx,vy,vz), initial row first. */
+void oracle_trajectory_coordtime(double a, const double y0[7], double h, int64_t nsteps, int64_t stride, double *out)
+{
+  double t = y0[0], y[6];
+  memcpy(y, y0 + 1, sizeof y);
+  out[0] = t; memcpy(out + 1, y, sizeof y);
+  int64_t rec = 1;
+  for (int64_t s = 1; s <= nsteps; ++s) {
+    oracle_rk4_step_coordtime(a, y, h);
+    t = y0[0] + (double)s * h;
+    if (s % stride == 0) { out[7 * rec] = t; memcpy(out + 7 * rec + 1, y, sizeof y); ++rec; }
+  }
+}
+
+int oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
+                               const oracle_step_control *sc, oracle_stats *stats)
+{
+  if (!s || !sc || n == 0 || n > s->n) return 1;
+  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return 1;
+  if (sc->dir != 1 && sc->dir != -1) return 1;
+  uint64_t steps = 0, nc = 0, ne = 0, nm = 0, ni = 0, na = 0;
+  const double a = s->a_eff, r_plus = 1.0 + sqrt(1.0 - a * a), dir = (double)sc->dir;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : steps, nc, ne, nm, ni, na)
+  for (int64_t k = 0; k < (int64_t)n; ++k) {
+    int32_t st = s->status[k], ns = s->nsteps[k], ns0 = ns;
+    if (st == ORACLE_ACTIVE) {
+      double t = s->q[0][k], y[6];
+      for (int i = 0; i < 3; ++i) { y[i] = s->q[1 + i][k]; y[3 + i] = s->q[5 + i][k] / s->q[4][k]; }
+      for (;;) {
+        double r = oracle_ks_r(a, y[0], y[1], y[2]);
+        int fin = isfinite(r) && isfinite(t);
+        for (int i = 0; i < 6; ++i) fin = fin && isfinite(y[i]);
+        if (!fin) { st = ORACLE_INVALID; break; }
+        if (r < sc->capture_factor * r_plus) { st = ORACLE_CAPTURED; break; }
+        if (r > sc->r_escape) { st = ORACLE_ESCAPED; break; }
+        if (ns >= sc->max_steps) { st = ORACLE_MAXSTEPS; break; }
+        if (dir * (t_end - t) <= 0.0) break;
+        double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
+        if (fabs(h) > fabs(t_end - t)) h = t_end - t;
+        oracle_rk4_step_coordtime(a, y, h);
+        t += h;
+        ns += 1;
+      }
+      s->q[0][k] = t;
+      for (int i = 0; i < 3; ++i) { s->q[1 + i][k] = y[i]; s->q[5 + i][k] = y[3 + i]; }
+      s->q[4][k] = 1.0;
+      s->status[k] = st; s->nsteps[k] = ns;
+    }
+    steps += (uint64_t)(ns - ns0);
+    nc += (st == ORACLE_CAPTURED); ne += (st == ORACLE_ESCAPED); nm += (st == ORACLE_MAXSTEPS);
+    ni += (st == ORACLE_INVALID);  na += (st == ORACLE_ACTIVE);
+  }
+  if (stats) {
+    stats->steps = steps; stats->n_captured = nc; stats->n_escaped = ne;
+    stats->n_maxsteps = nm; stats->n_invalid = ni; stats->n_active = na;
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
  * C8.  Independent Boyer-Lindquist integrator (oracle self-check only).
  * PAPER.md:47 eq. (1), M = 1, coordinates X = (t, r, theta, phi):
  *   ds^2 = -(1 - 2r/rho^2) dt^2 - (4 r a sin^2/rho^2) dphi dt + (rho^2/Delta) dr^2 + rho^2 dtheta^2

@@ -73,6 +73,16 @@ void   oracle_invariants_one(double a, int32_t kind, const double y[8], double o
    out has (nsteps/stride + 1) * 8 doubles. */
 void   oracle_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out);
 
+/* ---- coordinate-time form (eq. 15): six variables, v^mu = dx^mu/dt, v^0 = 1 ---- */
+void   oracle_ks_coordtime_accel(double a, const double pos[3], const double v[3], double dv[3]);  /* eq. (15) */
+void   oracle_rk4_step_coordtime(double a, double y[6], double h);                 /* y = x,y,z,vx,vy,vz */
+void   oracle_trajectory_coordtime(double a, const double y0[7], double h, int64_t nsteps, int64_t stride,
+                                   double *out);                                    /* rows t,x,y,z,vx,vy,vz */
+/* same driver loop as oracle_integrate with t in the role of lambda: stops at t_end (stays ACTIVE).
+   On entry v^i = q[5+i]/q[4]; on exit q[4] = 1, q[5..7] = v^i; `lambda` is not touched. */
+int    oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
+                                  const oracle_step_control *sc, oracle_stats *stats);
+
 /* ---- independent Boyer-Lindquist integrator (self-check only; eq. 1) ---- */
 void   oracle_bl_metric(double a, const double X[4], double g[16]);                 /* X = t,r,theta,phi  */
 void   oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4]);

@@ -13,7 +13,10 @@ import numpy as np
 import torch
 
 import oracle
+from paper_1706_07062_b200 import build as _build
 from paper_1706_07062_b200 import gray2
+
+_build.build()   # in-tree nvcc build; a no-op when libgray2.so is newer than its sources
 
 INF = float("inf")
 TOL_STATE_F64 = 1e-9
