@@ -178,7 +178,9 @@ def run_gpu(args):
 
     cfg = workload_config(args.workload)
     prec = gray2.F64 if args.dtype == "f64" else gray2.F32
-    flops_per_step = gray2.flops_per_step(prec)
+    coord = args.form == "coordtime"
+    flops_per_step = gray2.flops_per_step_coordtime(prec) if coord else gray2.flops_per_step(prec)
+    integrate = gray2.integrate_coordtime if coord else gray2.integrate
     props = torch.cuda.get_device_properties(local)
     n_sms = props.multi_processor_count
     peaks = load_measured_peaks()
@@ -197,7 +199,7 @@ def run_gpu(args):
         if ev: ev[0].record(stream)
         gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st)
         if ev: ev[1].record(stream)
-        gray2.integrate(st, INF, sc, stats=stats)
+        integrate(st, INF, sc, stats=stats)
         if ev: ev[2].record(stream)
         inv = gray2.invariants(st)
         if ev: ev[3].record(stream)
@@ -248,7 +250,7 @@ def run_gpu(args):
     def e2e_step():
         gray2.init_timelike(a_eff, host_in.numpy(), prec=prec, out=st)      # H2D inside (explicit 8-vectors)
         st.kind, st.reversed = gray2.NULL, 1
-        gray2.integrate(st, INF, sc, stats=stats)
+        integrate(st, INF, sc, stats=stats)
         inv = gray2.invariants(st)
         host_q.copy_(st.q, non_blocking=True); host_lam.copy_(st.lam, non_blocking=True)
         host_status.copy_(st.status, non_blocking=True); host_nsteps.copy_(st.nsteps, non_blocking=True)
@@ -294,13 +296,13 @@ def run_gpu(args):
             "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
             "config": {"workload": cfg.name, "rays_per_gpu": cfg.n, "rk4_steps_per_pass": steps_total // args.steps,
                        "a": cfg.a, "r_obs": cfg.r_obs, "inclination_deg": cfg.inclination_deg, "fov_half": cfg.fov,
-                       "step_rule": "dlambda = %g r" % cfg.eta, "l2": "flushed between timed iterations (256 MiB fill)",
+                       "form": args.form, "step_rule": ("dt = %g r" if coord else "dlambda = %g r") % cfg.eta, "l2": "flushed between timed iterations (256 MiB fill)",
                        "parallelism": "independent image per GPU, no collective"},
             "clocks": clocks,
             "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "gray2_init_timelike(host 8-vectors) -> gray2_integrate -> gray2_invariants -> D2H of state, invariants, stats"},
             "gpu_launches": 4 * args.steps,
-            "roofline": {"bound": "alu", "kernel": "integrate_kernel<%s>" % ("double" if prec == gray2.F64 else "float"),
+            "roofline": {"bound": "alu", "kernel": "integrate_kernel<%s%s>" % ("double" if prec == gray2.F64 else "float", ", coordinate time" if coord else ""),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": None, "flops_per_rk4_step": flops_per_step,
                          "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,
@@ -326,6 +328,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--form", default="affine", choices=["affine", "coordtime"],
+                    help="affine: gray2_integrate (eq. 13-14); coordtime: gray2_integrate_coordtime (eq. 18)")
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg5"])
     ap.add_argument("--oracle-side", type=int, default=128, help="oracle sample: side x side rays of the same field of view")
     ap.add_argument("--threads", type=int, default=0)

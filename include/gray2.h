@@ -103,6 +103,17 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
 int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
                     int32_t prec, gray2_stats *device_stats, void *cuda_stream);
 
+/* Coordinate-time form (section 2.2; eq. 18): integrates dv^i/dt = xddot^i - xddot^0 v^i,
+ * v^mu = dx^mu/dt with v^0 = 1, six variables, with the same classic RK4 and the same step and stopping
+ * rule as gray2_integrate, the KS coordinate time t = q[0] playing the role of lambda: the step is
+ * dt = dir * (mode == 1 ? eta * r : h_fixed), clipped so that t does not pass t_end, and a geodesic that
+ * reaches t_end stays ACTIVE ("integrate to a target KS coordinate time", method i).
+ * On entry v^i = q[5+i] / q[4]; on exit q[0] = t, q[4] = 1 and q[5..7] = v^i (DESIGN R19): a tangent
+ * vector of the same curve with another normalisation, so ratios such as L_z/E and Q/E^2 from
+ * gray2_invariants keep their meaning.  s->lambda is not touched.  device_stats as for gray2_integrate. */
+int gray2_integrate_coordtime(gray2_state *s, uint64_t n, double t_end, const gray2_step_control *sc,
+                              int32_t prec, gray2_stats *device_stats, void *cuda_stream);
+
 /* Constants of the RUN geodesic, always evaluated in double from the stored state (DESIGN R8):
  *   norm = g_ab u^a u^b ;  E = -u_t ;  L_z = x u_y - y u_x ;
  *   Q = u_theta^2 + cos^2(theta) [ a^2 (mu^2 - E^2) + L_z^2 / sin^2(theta) ], mu^2 nominal from s->kind.
@@ -117,6 +128,7 @@ int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per
 /* Exact floating-point operation counts of one RK4 step of one geodesic in this library's code path
  * (FMA = 2 flops, add/mul = 1, each rsqrt/rcp = 1), used for the roofline figure; see DESIGN.md. */
 int gray2_flops_per_step(int32_t prec);
+int gray2_flops_per_step_coordtime(int32_t prec);
 
 /* Diagnostic entry, not one of the four calls of the path: the geodesic right-hand side of eq. (13)-(14)
  * alone, at n points, so that tests can compare it element by element with the oracle's eq. (7).

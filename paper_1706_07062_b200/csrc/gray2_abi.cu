@@ -80,7 +80,7 @@ int check_state(const gray2_state *s, const char *who) {
 // ---- integrator dispatch ----------------------------------------------------------------------------
 namespace {
 
-template <typename T, int THREADS, int MIN_BLOCKS>
+template <typename T, int THREADS, int MIN_BLOCKS, int FORM>
 cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::StepParams<T> &p,
                              unsigned long long *queue, unsigned long long *steps, cudaStream_t st) {
   uint64_t want = (n + THREADS - 1) / THREADS;
@@ -88,33 +88,38 @@ cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::Step
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<T>(s);
   if (p.mode == 1) {
-    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
-    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
   } else {
-    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
-    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
   }
   return cudaGetLastError();
 }
 
 struct LaunchChoice { int threads, blocks; };
 
-// compiled variants; the first entry of each list is the default
-constexpr int kNumVariants = 5;
-constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}, {128, 2}, {256, 1}};
-constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 8}, {128, 6}, {256, 3}, {128, 4}, {128, 3}};
+// compiled variants of the affine-parameter integrator; the first entry of each list is the default,
+// and the only one compiled for the coordinate-time form
+constexpr int kNumVariants = 3;
+constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}};
+constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 8}, {128, 6}, {256, 3}};
 
 template <typename T>
-cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, uint64_t n,
+cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_state *s, uint64_t n,
                                const gray2::StepParams<T> &p, unsigned long long *q, unsigned long long *steps,
                                cudaStream_t st, bool *found) {
   *found = true;
+  if (form == 1) {
+    if constexpr (sizeof(T) == 8) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, st);
+    else return launch_integrate<T, 128, 8, 1>(s, n, p, q, steps, st);
+  }
 #define GRAY2_VARIANT(TH, BL) \
-  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL>(s, n, p, q, steps, st);
+  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
   if constexpr (sizeof(T) == 8) {
-    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(128, 2) GRAY2_VARIANT(256, 1)
+    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6)
   } else {
-    GRAY2_VARIANT(128, 6) GRAY2_VARIANT(128, 8) GRAY2_VARIANT(256, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(128, 3)
+    GRAY2_VARIANT(128, 8) GRAY2_VARIANT(128, 6) GRAY2_VARIANT(256, 3)
   }
 #undef GRAY2_VARIANT
   *found = false;
@@ -122,7 +127,7 @@ cudaError_t dispatch_integrate(int threads, int blocks, const gray2_state *s, ui
 }
 
 template <typename T>
-int integrate_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
                    gray2_stats *device_stats, cudaStream_t st) {
   const double a = s->a_eff;
   gray2::StepParams<T> p;
@@ -149,7 +154,7 @@ int integrate_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_st
   int threads = g_threads[pi] ? g_threads[pi] : def.threads;
   int blocks = g_blocks_per_sm[pi] ? g_blocks_per_sm[pi] : def.blocks;
   bool found = false;
-  cudaError_t e = dispatch_integrate<T>(threads, blocks, s, n, p, queue, steps, st, &found);
+  cudaError_t e = dispatch_integrate<T>(form, threads, blocks, s, n, p, queue, steps, st, &found);
   if (!found) return fail(GRAY2_EINVAL, "gray2_integrate: no compiled variant for %d threads x %d blocks/SM", threads, blocks);
   if (e != cudaSuccess) return fail(GRAY2_ECUDA, "integrate_kernel launch: %s", cudaGetErrorString(e));
 
@@ -220,25 +225,35 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
   return GRAY2_OK;
 }
 
-int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
-                    int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
-  int rc = check_state(s, "gray2_integrate");
+static int integrate_common(int form, const char *who, gray2_state *s, uint64_t n, double end,
+                            const gray2_step_control *sc, int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
+  int rc = check_state(s, who);
   if (rc) return rc;
-  if (!sc) return fail(GRAY2_EINVAL, "gray2_integrate: step control is NULL");
-  if (n == 0) return fail(GRAY2_EINVAL, "gray2_integrate: n == 0");
-  if (n > s->n) return fail(GRAY2_ESTATE, "gray2_integrate: n (%llu) exceeds s->n (%llu)", (unsigned long long)n, (unsigned long long)s->n);
-  if (prec != s->prec) return fail(GRAY2_EINVAL, "gray2_integrate: prec (%d) differs from s->prec (%d)", prec, s->prec);
-  if (sc->mode != 0 && sc->mode != 1) return fail(GRAY2_EINVAL, "gray2_integrate: mode must be 0 or 1");
-  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return fail(GRAY2_EINVAL, "gray2_integrate: step size must be > 0");
-  if (sc->dir != 1 && sc->dir != -1) return fail(GRAY2_EINVAL, "gray2_integrate: dir must be +1 or -1");
-  if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(lambda_end) || sc->max_steps < 0)
-    return fail(GRAY2_EINVAL, "gray2_integrate: bad capture_factor / r_escape / lambda_end / max_steps");
-  if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_integrate: |a_eff| must be <= 1");
+  if (!sc) return fail(GRAY2_EINVAL, "%s: step control is NULL", who);
+  if (n == 0) return fail(GRAY2_EINVAL, "%s: n == 0", who);
+  if (n > s->n) return fail(GRAY2_ESTATE, "%s: n (%llu) exceeds s->n (%llu)", who, (unsigned long long)n, (unsigned long long)s->n);
+  if (prec != s->prec) return fail(GRAY2_EINVAL, "%s: prec (%d) differs from s->prec (%d)", who, prec, s->prec);
+  if (sc->mode != 0 && sc->mode != 1) return fail(GRAY2_EINVAL, "%s: mode must be 0 or 1", who);
+  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return fail(GRAY2_EINVAL, "%s: step size must be > 0", who);
+  if (sc->dir != 1 && sc->dir != -1) return fail(GRAY2_EINVAL, "%s: dir must be +1 or -1", who);
+  if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(end) || sc->max_steps < 0)
+    return fail(GRAY2_EINVAL, "%s: bad capture_factor / r_escape / end value / max_steps", who);
+  if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a_eff| must be <= 1", who);
   rc = ensure_scratch();
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  return prec == GRAY2_F64 ? integrate_impl<double>(s, n, lambda_end, sc, device_stats, st)
-                           : integrate_impl<float>(s, n, lambda_end, sc, device_stats, st);
+  return prec == GRAY2_F64 ? integrate_impl<double>(form, s, n, end, sc, device_stats, st)
+                           : integrate_impl<float>(form, s, n, end, sc, device_stats, st);
+}
+
+int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                    int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
+  return integrate_common(0, "gray2_integrate", s, n, lambda_end, sc, prec, device_stats, cuda_stream);
+}
+
+int gray2_integrate_coordtime(gray2_state *s, uint64_t n, double t_end, const gray2_step_control *sc,
+                              int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
+  return integrate_common(1, "gray2_integrate_coordtime", s, n, t_end, sc, prec, device_stats, cuda_stream);
 }
 
 int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm,
@@ -280,6 +295,9 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
  *   radius 16, rest of geometry 24, velocity part 73  ->  113 per right-hand side
  *   4 x 113 + RK4 combination 100 + step rule and lambda update 2 = 554 per step (both precisions). */
 int gray2_flops_per_step(int32_t prec) { (void)prec; return 554; }
+
+/* Coordinate-time form: 4 x (113 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
+int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 558; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.

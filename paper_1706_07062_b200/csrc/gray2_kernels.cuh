@@ -90,7 +90,10 @@ __global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ 
 // every lane of the warp by one RK4 step per pass and leaves as soon as ANY lane's stopping test fires
 // (one vote per step).  In the hot path the stopping rule of gray2_step_control costs four compares:
 // the tests are ordered only in the (rare) slow path that classifies and stores a finished ray.
-template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP>
+//
+// FORM: 0 affine parameter (eq. 13-14, eight variables); 1 coordinate time (eq. 18, six variables): the
+// clock `lam` is then t itself, v^i = u^i/u^t on load, and (t, x, 1, v) is stored; `lambda` is untouched.
+template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long *queue,
                  unsigned long long *steps_out) {
@@ -124,7 +127,13 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
           idx = mine;
           ray.t = s.q[0][idx]; ray.x = s.q[1][idx]; ray.y = s.q[2][idx]; ray.z = s.q[3][idx];
           ray.u0 = s.q[4][idx]; ray.u1 = s.q[5][idx]; ray.u2 = s.q[6][idx]; ray.u3 = s.q[7][idx];
-          lam = s.lambda[idx];
+          if constexpr (FORM == 1) {
+            lam = (double)ray.t;
+            T w = fastmath<T>::rcp(ray.u0);
+            ray.u1 *= w; ray.u2 *= w; ray.u3 *= w; ray.u0 = T(1);
+          } else {
+            lam = s.lambda[idx];
+          }
           nst = nst0 = s.nsteps[idx];
           have = true;
         }
@@ -150,9 +159,11 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
           else if (g.r < p.r_capture) st = GRAY2_CAPTURED;
           else if (g.r > p.r_escape) st = GRAY2_ESCAPED;
           else if (nst >= p.max_steps) st = GRAY2_MAXSTEPS;
+          if constexpr (FORM == 1) ray.t = (T)lam;
           s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
           s.q[4][idx] = ray.u0; s.q[5][idx] = ray.u1; s.q[6][idx] = ray.u2; s.q[7][idx] = ray.u3;
-          s.lambda[idx] = lam; s.status[idx] = st; s.nsteps[idx] = nst;
+          if constexpr (FORM == 0) s.lambda[idx] = lam;
+          s.status[idx] = st; s.nsteps[idx] = nst;
           my_steps += (unsigned long long)(nst - nst0);
           have = false;
         }
@@ -164,7 +175,8 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
         double rem = p.lambda_end - lam;
         if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
       }
-      rk4_step(k, ray, g, h);
+      if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
+      else rk4_step(k, ray, g, h);
       lam += hd;
       nst += 1;
     }

@@ -220,4 +220,47 @@ __device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const
   s.u3 = fma_(h6, S3 + b3, s.u3);
 }
 
+// ---- coordinate-time form ------------------------------------------------------
+// v^mu = dx^mu/dt, v^0 = 1.  PAPER.md:146 eq. (18): the right-hand side is the affine one evaluated with
+// u = (1, v) and recombined,  dv^i/dt = xddot^i - xddot^0 v^i  -- "the same computational complexity".
+template <typename T>
+__device__ __forceinline__ void ks_accel_coordtime(const SpinConst<T> &k, const Geometry<T> &g, T x, T y,
+                                                   T v1, T v2, T v3, T &d1, T &d2, T &d3) {
+  T a0, a1, a2, a3;
+  ks_accel(k, g, x, y, T(1), v1, v2, v3, a0, a1, a2, a3);
+  d1 = fma_(-a0, v1, a1);
+  d2 = fma_(-a0, v2, a2);
+  d3 = fma_(-a0, v3, a3);
+}
+
+// Classic RK4 in t of the six variables (x, v); uses Ray<T> with u0 unused (v^0 = 1) and t advanced by
+// the caller (t += h exactly).
+template <typename T>
+__device__ __forceinline__ void rk4_step_coordtime(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, T h) {
+  const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
+  T b1, b2, b3, v1, v2, v3, px, py, pz;
+  T Sx, Sy, Sz, S1, S2, S3;
+  Geometry<T> g;
+  ks_accel_coordtime(k, g1, s.x, s.y, s.u1, s.u2, s.u3, b1, b2, b3);
+  Sx = s.u1; Sy = s.u2; Sz = s.u3; S1 = b1; S2 = b2; S3 = b3;
+  px = fma_(hh, s.u1, s.x); py = fma_(hh, s.u2, s.y); pz = fma_(hh, s.u3, s.z);
+  v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
+  ks_geometry(k, px, py, pz, g);
+  ks_accel_coordtime(k, g, px, py, v1, v2, v3, b1, b2, b3);
+  Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
+  S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
+  px = fma_(hh, v1, s.x); py = fma_(hh, v2, s.y); pz = fma_(hh, v3, s.z);
+  v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
+  ks_geometry(k, px, py, pz, g);
+  ks_accel_coordtime(k, g, px, py, v1, v2, v3, b1, b2, b3);
+  Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
+  S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
+  px = fma_(h, v1, s.x); py = fma_(h, v2, s.y); pz = fma_(h, v3, s.z);
+  v1 = fma_(h, b1, s.u1); v2 = fma_(h, b2, s.u2); v3 = fma_(h, b3, s.u3);
+  ks_geometry(k, px, py, pz, g);
+  ks_accel_coordtime(k, g, px, py, v1, v2, v3, b1, b2, b3);
+  s.x = fma_(h6, Sx + v1, s.x); s.y = fma_(h6, Sy + v2, s.y); s.z = fma_(h6, Sz + v3, s.z);
+  s.u1 = fma_(h6, S1 + b1, s.u1); s.u2 = fma_(h6, S2 + b2, s.u2); s.u3 = fma_(h6, S3 + b3, s.u3);
+}
+
 }  // namespace gray2

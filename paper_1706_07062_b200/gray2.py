@@ -67,6 +67,10 @@ def load_library():
     lib.gray2_init_null.argtypes = [p, d, d, d, d, d, i32, i32, p]
     lib.gray2_init_timelike.argtypes = [p, d, p, u64, i32, p]
     lib.gray2_integrate.argtypes = [p, u64, d, p, i32, p, p]
+    lib.gray2_integrate_coordtime.argtypes = [p, u64, d, p, i32, p, p]
+    lib.gray2_integrate_coordtime.restype = C.c_int
+    lib.gray2_flops_per_step_coordtime.argtypes = [i32]
+    lib.gray2_flops_per_step_coordtime.restype = C.c_int
     lib.gray2_invariants.argtypes = [p, u64, p, p, p, p, p]
     lib.gray2_rhs.argtypes = [i32, d, u64, p, p, p, p]
     lib.gray2_set_launch.argtypes = [i32, i32, i32]
@@ -172,6 +176,17 @@ def integrate(st: State, lambda_end, sc: StepControl, n=None, stats: torch.Tenso
     return stats
 
 
+def integrate_coordtime(st: State, t_end, sc: StepControl, n=None, stats: torch.Tensor | None = None, stream=None):
+    """Coordinate-time form (paper eq. 18): advance every ACTIVE geodesic to KS time t_end (see gray2.h)."""
+    cs = st._c()
+    sp = C.c_void_p(stats.data_ptr()) if stats is not None else C.c_void_p(0)
+    if stats is not None:
+        assert stats.is_cuda and stats.dtype == torch.int64 and stats.numel() >= 6
+    _check(load_library().gray2_integrate_coordtime(C.byref(cs), st.n if n is None else n, float(t_end),
+                                                    C.byref(sc), st.prec, sp, _stream_ptr(stream)))
+    return stats
+
+
 def new_stats(device="cuda") -> torch.Tensor:
     return torch.zeros(6, dtype=torch.int64, device=device)
 
@@ -217,6 +232,10 @@ def set_launch(prec, threads_per_block=0, blocks_per_sm=0):
 
 def flops_per_step(prec=F64) -> int:
     return int(load_library().gray2_flops_per_step(prec))
+
+
+def flops_per_step_coordtime(prec=F64) -> int:
+    return int(load_library().gray2_flops_per_step_coordtime(prec))
 
 
 def version() -> str:
