@@ -16,7 +16,7 @@
 //             B = [[r/P, -a/P, 0], [a/P, r/P, 0], [0, 0, 1/r]]
 //
 // The 12 elements xdot_{beta,alpha} = g_{beta gamma,alpha} xdot^gamma of PAPER.md:100 never need to be
-// stored: with U = u0 + l.u they collapse to
+// stored: with U = u0 + l.u they collapse to (ks_accel below uses a further regrouping of the same terms)
 //   omega = curl l = grad r x A + (0, 0, -2a/P)                 (antisymmetric part of d_j l_i)
 //   q     = u_i u_j d_j l_i = (u.grad r)(A.u) + (r/P)(u1^2+u2^2) + u3^2 / r   (symmetric part)
 //   l.grad f = f (c1 - c2 l3)       because l.grad r = 1 and (l.grad) l = 0 (l is a geodesic null field)
@@ -51,7 +51,6 @@ template <> struct fastmath<double> {
     double t = fma(e, e, e);                   // y <- y (1 + e + e^2)
     return fma(y, t, y);
   }
-  static __device__ __forceinline__ double sqrt_ieee(double x) { return ::sqrt(x); }
   static __device__ __forceinline__ bool finite(double x) { return fabs(x) <= 1.7976931348623157e308; }
 };
 
@@ -66,7 +65,6 @@ template <> struct fastmath<float> {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
   }
-  static __device__ __forceinline__ float sqrt_ieee(float x) { return ::sqrtf(x); }
   static __device__ __forceinline__ bool finite(float x) { return fabsf(x) <= 3.402823466e38f; }
 };
 

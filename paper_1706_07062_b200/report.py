@@ -137,9 +137,42 @@ def report_cfg4(n, nsteps):
                 generator_seconds=gen_s, acceptance=meta["acceptance"], drift_of_particles_still_orbiting=drift)
 
 
+def report_paper_benchmark():
+    """The paper's own benchmark shape: null geodesics traced back from an image at
+    r = 1024 M toward a = 0.999, fixed step, 1024 RK4 steps per call, calls repeated until every ray is
+    captured or has escaped beyond its initial radius; image sizes 64^2 ... 1024^2; reported: the
+    shortest call time divided by the steps it executed = ns per RK4 step per ray (Table 2's unit).
+    The paper does not state step size, inclination or field of view: h = 1/32 (64 calls x 1024 steps
+    cover the 2 x 1024 M path), i = 60 deg, +-15 M are used here."""
+    out = {}
+    for prec, name in ((gray2.F64, "double"), (gray2.F32, "single")):
+        best = {}
+        for side in (64, 128, 256, 512, 1024):
+            st = gray2.init_null(0.999, 1024.0, math.radians(60.0), 15.0, 15.0, side, side, prec=prec)
+            stats = gray2.new_stats()
+            calls, best_ns, total_steps = 0, float("inf"), 0
+            while True:
+                calls += 1
+                sc = gray2.step_control(mode=0, h_fixed=1.0 / 32.0, r_escape=1024.5, max_steps=1024 * calls)
+                _, dt = _timed(lambda: gray2.integrate(st, INF, sc, stats=stats))
+                sd = gray2.stats_dict(stats)
+                total_steps += sd["steps"]
+                if sd["steps"] > 0.5 * 1024 * side * side:           # launches that still step most rays
+                    best_ns = min(best_ns, 1e9 * dt / sd["steps"])
+                if sd["n_maxsteps"] == 0 or calls >= 80:
+                    break
+                st.status[st.status == gray2.MAXSTEPS] = gray2.ACTIVE   # continue the unfinished rays
+            best[str(side)] = {"calls": calls, "best_ns_per_step_per_ray": best_ns, "total_steps": total_steps}
+        out[name] = {"per_image_size": best,
+                     "ns_per_step_per_ray": min(v["best_ns_per_step_per_ray"] for v in best.values())}
+    out["paper_table2_KS_SoA_best"] = {"single": "0.309 ns (Titan Black)", "double": "1.15 ns (Titan Black)",
+                                       "cite": "PAPER.md:286-288"}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", default="1,2,3,4,5")
+    ap.add_argument("--configs", default="1,2,3,4,5", help="comma list of 1..5 and P (the paper's benchmark shape)")
     ap.add_argument("--cfg4-steps", type=int, default=100000)
     ap.add_argument("--cfg4-n", type=int, default=1 << 20)
     args = ap.parse_args()
@@ -157,6 +190,8 @@ def main():
         out["cfg5"] = {"f32": run_image(inputs.CFG5_NULL, gray2.F32)[1]}
         torch.cuda.empty_cache()
         out["cfg5"]["f64"] = run_image(inputs.CFG5_NULL, gray2.F64)[1]
+    if "P" in want:
+        out["paper_benchmark"] = report_paper_benchmark()
     print(json.dumps(out, indent=1))
 
 
