@@ -19,7 +19,7 @@ DEPS = SOURCES + [os.path.join(CSRC, "gray2_kernels.cuh"), os.path.join(CSRC, "k
                   os.path.join(os.path.dirname(HERE), "include", "gray2.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--fmad=true",
+              "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--fmad=false",
               "-Xptxas", "-v,-warn-spills"]
 
 

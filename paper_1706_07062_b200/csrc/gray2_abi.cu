@@ -97,31 +97,56 @@ cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::Step
   return cudaGetLastError();
 }
 
+// FP32 with two geodesics per thread (packed FP32x2 arithmetic)
+template <int THREADS, int MIN_BLOCKS, int FORM>
+cudaError_t launch_integrate_x2(const gray2_state *s, uint64_t n, const gray2::StepParams<float> &p,
+                                unsigned long long *queue, unsigned long long *steps, cudaStream_t st) {
+  uint64_t want = (n + 2 * THREADS - 1) / (2 * THREADS);
+  uint64_t cap = (uint64_t)g_num_sms * MIN_BLOCKS;
+  unsigned grid = (unsigned)(want < cap ? want : cap);
+  auto v = view_of<float>(s);
+  if (p.mode == 1) {
+    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+  } else {
+    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+  }
+  return cudaGetLastError();
+}
+
 struct LaunchChoice { int threads, blocks; };
 
-// compiled variants of the affine-parameter integrator; the first entry of each list is the default,
-// and the only one compiled for the coordinate-time form
-constexpr int kNumVariants = 3;
-constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}};
-constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 8}, {128, 6}, {256, 3}};
+// Compiled variants of the affine-parameter integrator; the first entry of each list is the default
+// and the only one compiled for the coordinate-time form.  FP32: the first three entries run two
+// geodesics per thread (integrate_kernel_f32x2), the last two one per thread (integrate_kernel<float>);
+// every variant gives bit-identical results.
+constexpr int kNumVariants = 5;
+constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}, {256, 1}, {128, 2}};
+constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 4}, {128, 3}, {256, 2}, {128, 8}, {128, 6}};
 
 template <typename T>
 cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_state *s, uint64_t n,
                                const gray2::StepParams<T> &p, unsigned long long *q, unsigned long long *steps,
                                cudaStream_t st, bool *found) {
   *found = true;
-  if (form == 1) {
-    if constexpr (sizeof(T) == 8) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, st);
-    else return launch_integrate<T, 128, 8, 1>(s, n, p, q, steps, st);
-  }
+  if constexpr (sizeof(T) == 8) {
+    if (form == 1) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
-  if constexpr (sizeof(T) == 8) {
-    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6)
-  } else {
-    GRAY2_VARIANT(128, 8) GRAY2_VARIANT(128, 6) GRAY2_VARIANT(256, 3)
-  }
+    GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(128, 2)
 #undef GRAY2_VARIANT
+  } else {
+    if (form == 1) return launch_integrate_x2<128, 4, 1>(s, n, p, q, steps, st);
+#define GRAY2_VARIANT_X2(TH, BL) \
+  if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, st);
+#define GRAY2_VARIANT(TH, BL) \
+  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
+    GRAY2_VARIANT_X2(128, 4) GRAY2_VARIANT_X2(128, 3) GRAY2_VARIANT_X2(256, 2)
+    GRAY2_VARIANT(128, 8) GRAY2_VARIANT(128, 6)
+#undef GRAY2_VARIANT
+#undef GRAY2_VARIANT_X2
+  }
   *found = false;
   return cudaSuccess;
 }
@@ -292,12 +317,12 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
 }
 
 /* Source-level count of ks_geodesic.cuh (FMA = 2, add/mul = 1, rsqrt/rcp = 1; negations and compares free):
- *   radius 16, rest of geometry 24, velocity part 73  ->  113 per right-hand side
- *   4 x 113 + RK4 combination 100 + step rule and lambda update 2 = 554 per step (both precisions). */
-int gray2_flops_per_step(int32_t prec) { (void)prec; return 554; }
+ *   radius 16, rest of geometry 23, velocity part 75  ->  114 per right-hand side
+ *   4 x 114 + RK4 combination 100 + step rule and lambda update 2 = 558 per step (both precisions). */
+int gray2_flops_per_step(int32_t prec) { (void)prec; return 558; }
 
-/* Coordinate-time form: 4 x (113 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
-int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 558; }
+/* Coordinate-time form: 4 x (114 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
+int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 562; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.

@@ -12,6 +12,7 @@
 #include <stdint.h>
 #include "../../include/gray2.h"
 #include "ks_geodesic.cuh"
+#include "f32x2.cuh"
 
 namespace gray2 {
 
@@ -183,6 +184,126 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
   }
 
   // ---- per-warp reduction of the step count -----------------------------------------------------
+  for (int off = 16; off > 0; off >>= 1) my_steps += __shfl_down_sync(0xffffffffu, my_steps, off);
+  if (lane == 0 && my_steps) atomicAdd(steps_out, my_steps);
+}
+
+// ---- FP32, two geodesics per thread (packed FP32x2 arithmetic, see f32x2.cuh) -----------------------
+// Same loop structure as integrate_kernel.  Each thread owns two slots (the halves of every register
+// pair); a warp therefore holds 64 geodesics, refilled slot by slot from the same queue.
+struct PairSlot {
+  uint64_t idx;
+  double lam;
+  int32_t nst, nst0;
+  bool have;
+};
+
+template <int C, int FORM>
+__device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, uint64_t mine, Ray<f32x2> &ray,
+                                          PairSlot &sl) {
+  if (mine < n && s.status[mine] == GRAY2_ACTIVE) {
+    sl.idx = mine;
+    float t = s.q[0][mine], u0 = s.q[4][mine], u1 = s.q[5][mine], u2 = s.q[6][mine], u3 = s.q[7][mine];
+    if (FORM == 1) {
+      sl.lam = (double)t;
+      float w = fastmath<float>::rcp(u0);
+      u1 *= w; u2 *= w; u3 *= w; u0 = 1.0f;
+    } else {
+      sl.lam = s.lambda[mine];
+    }
+    set_half<C>(ray.t, t); set_half<C>(ray.x, s.q[1][mine]); set_half<C>(ray.y, s.q[2][mine]);
+    set_half<C>(ray.z, s.q[3][mine]); set_half<C>(ray.u0, u0); set_half<C>(ray.u1, u1);
+    set_half<C>(ray.u2, u2); set_half<C>(ray.u3, u3);
+    sl.nst = sl.nst0 = s.nsteps[mine];
+    sl.have = true;
+  }
+}
+
+template <int C, bool CLIP>
+__device__ __forceinline__ bool slot_may_step(const StepParams<float> &p, const Geometry<f32x2> &g, f32x2 U,
+                                              const Ray<f32x2> &ray, const PairSlot &sl) {
+  float r = half_of<C>(g.r);
+  bool go = (r >= p.r_capture) && (r <= p.r_escape_fin) && fastmath<float>::finite(half_of<C>(U)) &&
+            fastmath<float>::finite(half_of<C>(ray.t)) && (sl.nst < p.max_steps);
+  if (CLIP) go = go && (p.dir * (p.lambda_end - sl.lam) > 0.0);
+  return go;
+}
+
+template <int C, int FORM>
+__device__ __forceinline__ void store_slot(const StateView<float> &s, const StepParams<float> &p,
+                                           const Geometry<f32x2> &g, f32x2 U, const Ray<f32x2> &ray, PairSlot &sl,
+                                           unsigned long long &my_steps) {
+  float r = half_of<C>(g.r), t = half_of<C>(ray.t);
+  int32_t st = GRAY2_ACTIVE;
+  if (!(fastmath<float>::finite(r) && fastmath<float>::finite(half_of<C>(U)) && fastmath<float>::finite(t))) st = GRAY2_INVALID;
+  else if (r < p.r_capture) st = GRAY2_CAPTURED;
+  else if (r > p.r_escape) st = GRAY2_ESCAPED;
+  else if (sl.nst >= p.max_steps) st = GRAY2_MAXSTEPS;
+  const uint64_t i = sl.idx;
+  s.q[0][i] = FORM == 1 ? (float)sl.lam : t;
+  s.q[1][i] = half_of<C>(ray.x); s.q[2][i] = half_of<C>(ray.y); s.q[3][i] = half_of<C>(ray.z);
+  s.q[4][i] = half_of<C>(ray.u0); s.q[5][i] = half_of<C>(ray.u1); s.q[6][i] = half_of<C>(ray.u2);
+  s.q[7][i] = half_of<C>(ray.u3);
+  if (FORM == 0) s.lambda[i] = sl.lam;
+  s.status[i] = st; s.nsteps[i] = sl.nst;
+  my_steps += (unsigned long long)(sl.nst - sl.nst0);
+  sl.have = false;
+}
+
+template <int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
+__global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
+integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsigned long long *queue,
+                       unsigned long long *steps_out) {
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const SpinConst<f32x2> k{f32x2(p.k.a), f32x2(p.k.a2), f32x2(p.k.two_a), f32x2(p.k.two_a2)};
+
+  Ray<f32x2> ray;
+  ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = f32x2(0.0f);
+  ray.z = f32x2(3.0f);         // idle slots integrate a harmless dummy state (never stored)
+  PairSlot A{0, 0.0, 0, 0, false}, B{0, 0.0, 0, 0, false};
+  bool drained = false;
+  unsigned long long my_steps = 0;
+
+  for (;;) {
+    unsigned idleA = __ballot_sync(0xffffffffu, !A.have), idleB = __ballot_sync(0xffffffffu, !B.have);
+    if ((idleA | idleB) && !drained) {
+      unsigned cntA = __popc(idleA), cnt = cntA + __popc(idleB);
+      unsigned long long base = 0;
+      if (lane == 0) base = atomicAdd(queue, (unsigned long long)cnt);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (base + cnt >= n) drained = true;
+      if (!A.have) load_slot<0, FORM>(s, n, base + __popc(idleA & lt_mask), ray, A);
+      if (!B.have) load_slot<1, FORM>(s, n, base + cntA + __popc(idleB & lt_mask), ray, B);
+      continue;
+    }
+    if ((idleA & idleB) == 0xffffffffu) break;
+
+    for (;;) {
+      Geometry<f32x2> g;
+      ks_geometry(k, ray.x, ray.y, ray.z, g);
+      f32x2 U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+      bool stopA = A.have && !slot_may_step<0, CLIP>(p, g, U, ray, A);
+      bool stopB = B.have && !slot_may_step<1, CLIP>(p, g, U, ray, B);
+      if (__any_sync(0xffffffffu, stopA || stopB)) {
+        if (stopA) store_slot<0, FORM>(s, p, g, U, ray, A, my_steps);
+        if (stopB) store_slot<1, FORM>(s, p, g, U, ray, B, my_steps);
+        break;
+      }
+      f32x2 h = (MODE == 1) ? f32x2(p.eta_or_h) * g.r : f32x2(p.eta_or_h);
+      double hdA = (double)h.v.x, hdB = (double)h.v.y;
+      if (CLIP) {
+        double remA = p.lambda_end - A.lam, remB = p.lambda_end - B.lam;
+        if (fabs(hdA) > fabs(remA)) { hdA = remA; h.v.x = (float)remA; }
+        if (fabs(hdB) > fabs(remB)) { hdB = remB; h.v.y = (float)remB; }
+      }
+      if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
+      else rk4_step(k, ray, g, h);
+      A.lam += hdA; B.lam += hdB;
+      A.nst += 1; B.nst += 1;
+    }
+  }
+
   for (int off = 16; off > 0; off >>= 1) my_steps += __shfl_down_sync(0xffffffffu, my_steps, off);
   if (lane == 0 && my_steps) atomicAdd(steps_out, my_steps);
 }

@@ -99,8 +99,7 @@ __device__ __forceinline__ void ks_radius(const SpinConst<T> &k, T x, T y, T z, 
   T b = k.two_a * z;
   T D2 = fma_(b, b, w * w);
   Dinv = fastmath<T>::rsqrt(D2);
-  T D = D2 * Dinv;
-  r2 = T(0.5) * (w + D);
+  r2 = T(0.5) * fma_(D2, Dinv, w);          // (w + D)/2 with D = D2 / sqrt(D2)
   rinv = fastmath<T>::rsqrt(r2);
   r = r2 * rinv;
 }
@@ -122,9 +121,10 @@ __device__ __forceinline__ void ks_geometry(const SpinConst<T> &k, T x, T y, T z
   g.zeta = z * (P * rinv2);
   T c1 = fma_(T(3), rinv, -(f + f));
   T c2 = k.two_a2 * z * (Dinv * rinv2);
-  g.alpha = (f * c1) * hf;
+  T fc1 = f * c1;
+  g.alpha = fc1 * hf;
   g.beta = c2 * f;
-  g.lf = f * fma_(-c2, g.l3, c1);
+  g.lf = fma_(-g.beta, g.l3, fc1);
   g.tr = r + r;
   g.trP = g.tr * Pinv;
   g.rP = r * Pinv;
@@ -137,9 +137,10 @@ __device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T
                                          T u0, T u1, T u2, T u3, T &a0, T &a1, T &a2, T &a3) {
   T xu = fma_(x, u1, y * u2);
   T yu = fma_(y, u1, -x * u2);
-  T lu = g.Pinv * fma_(g.r, xu, k.a * yu);        // l1 u1 + l2 u2
+  T Lu = fma_(g.r, xu, k.a * yu);
+  T lu = g.Pinv * Lu;                              // l1 u1 + l2 u2
   T zu = g.l3 * u3;
-  T U = (u0 + lu) + zu;                            // l_alpha u^alpha
+  T U = fma_(g.l3, u3, fma_(g.Pinv, Lu, u0));      // l_alpha u^alpha
   T Au = fma_(g.Pinv, fma_(-g.tr, lu, xu), -zu * g.rinv);
   T unv = fma_(g.zeta, u3, xu);                    // n . u
   T ur = g.hf * unv;                               // u . grad r
@@ -152,9 +153,8 @@ __device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T
   T cn = fma_(fU * g.hf, Au, hU2 * g.alpha);
   T cA = fU * ur;
   T cB = fU * g.taP;
-  T e1 = -cA * g.Pinv;
   T e2 = g.Pinv * fma_(cA, g.trP, -a0);
-  T kap = fma_(e2, g.r, cn + e1);
+  T kap = fma_(e2, g.r, fma_(-cA, g.Pinv, cn));
   T mu = e2 * k.a;
   a1 = fma_(kap, x, fma_(mu, y, -cB * u2));
   a2 = fma_(kap, y, fma_(-mu, x, cB * u1));
@@ -166,8 +166,8 @@ template <typename T>
 __device__ __forceinline__ T ks_U(const SpinConst<T> &k, const Geometry<T> &g, T x, T y, T u0, T u1, T u2, T u3) {
   T xu = fma_(x, u1, y * u2);
   T yu = fma_(y, u1, -x * u2);
-  T lu = g.Pinv * fma_(g.r, xu, k.a * yu);
-  return (u0 + lu) + g.l3 * u3;
+  T Lu = fma_(g.r, xu, k.a * yu);
+  return fma_(g.l3, u3, fma_(g.Pinv, Lu, u0));
 }
 
 // One geodesic's 8 variables.

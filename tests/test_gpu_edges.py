@@ -117,6 +117,25 @@ def test_results_do_not_depend_on_launch_shape_or_run():
         gray2.set_launch(gray2.F64, 0, 0)
 
 
+def test_fp32_packed_and_scalar_kernels_agree_bit_for_bit():
+    """FP32 runs two geodesics per thread with packed FP32x2 instructions by default; the one-per-thread
+    float kernel must give the same bits (every FMA is explicit, the library is built with --fmad=false)."""
+    cfg = inputs.CFG3_NULL.scaled(150, 91)          # odd ray count: the last thread has an empty second slot
+    ref = None
+    try:
+        for shape in [(0, 0), (128, 3), (256, 2), (128, 8), (128, 6)]:
+            gray2.set_launch(gray2.F32, *shape)
+            _, g, stats = run_gpu_image(cfg, prec=gray2.F32)
+            cur = (g.q.clone(), g.nsteps.clone(), g.status.clone(), g.lam.clone(), stats)
+            if ref is None:
+                ref = cur
+            else:
+                assert all(torch.equal(x, y) for x, y in zip(ref[:4], cur[:4])) and ref[4] == cur[4], shape
+    finally:
+        gray2.set_launch(gray2.F32, 0, 0)
+    assert ref[4]["n_active"] == 0 and ref[4]["n_captured"] + ref[4]["n_escaped"] == cfg.n
+
+
 def test_backward_direction_and_lambda_clip():
     xu8, _ = inputs.cfg4_ensemble(64)
     g = gray2.init_timelike(0.7, xu8)
