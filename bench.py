@@ -49,20 +49,23 @@ def load_measured_peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons during the timed region (profiling recipe)."""
+    """Samples nvidia-smi clocks and throttle reasons (profiling recipe).  It is started before the warm-up
+    so that nvidia-smi's start-up cost is not inside the timed region; every sample is stamped on arrival
+    and only the samples that fall inside the timed window are reported."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
 
     def __init__(self, index):
         self.index = index
-        self.lines = []
+        self.samples = []          # (arrival time, fields)
         self.proc = None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._pump, daemon=True).start()
         except Exception:
@@ -70,16 +73,22 @@ class ClockSampler:
 
     def _pump(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.samples.append((time.perf_counter(), line.strip()))
 
-    def stop(self) -> dict:
+    def wait_for_first_sample(self, timeout=3.0):
+        t0 = time.perf_counter()
+        while self.proc is not None and not self.samples and time.perf_counter() - t0 < timeout:
+            time.sleep(0.01)
+
+    def stop(self, t_begin, t_end) -> dict:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
+        time.sleep(0.05)
         self.proc.terminate()
         sm, smax, power, reasons = [], [], [], set()
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for ln in self.lines:
+        for stamp, ln in self.samples:
+            if not (t_begin <= stamp <= t_end + 0.03):
+                continue
             parts = [p.strip() for p in ln.split(",")]
             if len(parts) < 7:
                 continue
@@ -87,14 +96,13 @@ class ClockSampler:
                 sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
             except ValueError:
                 continue
-            for nm, val in zip(names, parts[3:7]):
+            for nm, val in zip(self.NAMES, parts[3:7]):
                 if val.lower().startswith("active"):
                     reasons.add(nm)
         if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
-        busy = [c for c, p in zip(sm, power) if p > 0.5 * max(power)] or sm
-        return {"sm_mhz": statistics.median(busy), "sm_max_mhz": max(smax), "power_w_max": max(power),
-                "samples": len(sm), "reasons": sorted(reasons)}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples inside the timed window"]}
+        return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "sm_max_mhz": max(smax),
+                "power_w_max": max(power), "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def workload_config(name: str):
@@ -205,19 +213,21 @@ def run_gpu(args):
         if ev: ev[3].record(stream)
         return inv
 
-    for _ in range(max(args.warmup, 3)):
-        one_step()
-    torch.cuda.synchronize()
-
     try:
         gpu_id = "GPU-" + str(props.uuid) if not str(props.uuid).startswith("GPU-") else str(props.uuid)
     except Exception:
         gpu_id = str(local)
     sampler = ClockSampler(gpu_id)
+    sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    torch.cuda.synchronize()
+    sampler.wait_for_first_sample()
+
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    sampler.start()
+    t_window0 = time.perf_counter()
     t_step, t_int, steps_total = 0.0, 0.0, 0
     for _ in range(args.steps):
         flush.fill_(1)                                     # flush L2 between timed iterations (untimed)
@@ -230,7 +240,7 @@ def run_gpu(args):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    clocks = sampler.stop()
+    clocks = sampler.stop(t_window0, time.perf_counter())
 
     # ---- end to end through the public API with HOST buffers (pinned): H2D of the 8-vectors, D2H of results
     host_in = torch.empty((cfg.n, 8), dtype=torch.float64).pin_memory()
@@ -302,7 +312,8 @@ def run_gpu(args):
             "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "gray2_init_timelike(host 8-vectors) -> gray2_integrate -> gray2_invariants -> D2H of state, invariants, stats"},
             "gpu_launches": 4 * args.steps,
-            "roofline": {"bound": "alu", "kernel": "integrate_kernel<%s%s>" % ("double" if prec == gray2.F64 else "float", ", coordinate time" if coord else ""),
+            "roofline": {"bound": "alu", "kernel": ("integrate_kernel<double%s>" if prec == gray2.F64 else "integrate_kernel_f32x2<%s>") % (
+                             ", coordinate time" if coord else ("" if prec == gray2.F64 else "affine")),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": None, "flops_per_rk4_step": flops_per_step,
                          "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,

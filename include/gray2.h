@@ -17,8 +17,8 @@
  *
  * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
  * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
- * library allocates no persistent memory of its own except one 64-byte work-queue scratch per process,
- * and temporary staging inside gray2_init_timelike (freed stream-ordered).  `host_xu8` is a HOST pointer.
+ * library allocates no device memory of its own except a 4 KiB work-queue scratch and the staging buffer
+ * of gray2_init_timelike (n x 64 bytes, grown on demand, reused, released at process exit).  `host_xu8` is a HOST pointer.
  * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
  *
  * Asynchrony.  Every call enqueues on `cuda_stream` (a cudaStream_t passed as void*, NULL = default

@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include <atomic>
+#include <mutex>
 
 #include "../../include/gray2.h"
 #include "gray2_kernels.cuh"
@@ -123,7 +124,7 @@ struct LaunchChoice { int threads, blocks; };
 // every variant gives bit-identical results.
 constexpr int kNumVariants = 5;
 constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}, {256, 1}, {128, 2}};
-constexpr LaunchChoice kF32Variants[kNumVariants] = {{128, 4}, {128, 3}, {256, 2}, {128, 8}, {128, 6}};
+constexpr LaunchChoice kF32Variants[kNumVariants] = {{256, 2}, {128, 3}, {128, 4}, {128, 8}, {128, 6}};
 
 template <typename T>
 cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_state *s, uint64_t n,
@@ -137,7 +138,7 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
     GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(128, 2)
 #undef GRAY2_VARIANT
   } else {
-    if (form == 1) return launch_integrate_x2<128, 4, 1>(s, n, p, q, steps, st);
+    if (form == 1) return launch_integrate_x2<256, 2, 1>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT_X2(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT(TH, BL) \
@@ -230,9 +231,19 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
   if (n > s->n) return fail(GRAY2_ESTATE, "gray2_init_timelike: n (%llu) exceeds s->n (%llu)", (unsigned long long)n, (unsigned long long)s->n);
   if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_timelike: |a| must be <= 1 (got %g)", a);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  double *stage = nullptr;
+  // Staging buffer for the AoS input: owned by the library, grown on demand and reused (a fresh
+  // stream-ordered allocation per call costs up to 100 ms when the pool has to grow again).  The lock is
+  // held until the stream has been synchronised, so concurrent callers cannot overwrite each other's input.
+  static std::mutex stage_lock;
+  static double *stage = nullptr;
+  static size_t stage_bytes = 0;
+  std::lock_guard<std::mutex> guard(stage_lock);
   size_t bytes = (size_t)n * 8 * sizeof(double);
-  CUDA_TRY(cudaMallocAsync(&stage, bytes, st));
+  if (bytes > stage_bytes) {
+    if (stage) { cudaFree(stage); stage = nullptr; stage_bytes = 0; }
+    CUDA_TRY(cudaMalloc(&stage, bytes));
+    stage_bytes = bytes;
+  }
   cudaError_t e = cudaMemcpyAsync(stage, host_xu8, bytes, cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) {
     unsigned grid = (unsigned)((n + 255) / 256);
@@ -242,9 +253,7 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
       gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), stage, n, a, renorm);
     e = cudaGetLastError();
   }
-  cudaError_t e2 = cudaFreeAsync(stage, st);
-  if (e == cudaSuccess) e = e2;
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // host_xu8 may be pageable: make reuse safe
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the staging buffer and host_xu8 may be reused on return
   if (e != cudaSuccess) return fail(GRAY2_ECUDA, "gray2_init_timelike: %s", cudaGetErrorString(e));
   s->a_eff = a; s->kind = GRAY2_TIMELIKE; s->reversed = 0;
   return GRAY2_OK;

@@ -123,7 +123,7 @@ def test_fp32_packed_and_scalar_kernels_agree_bit_for_bit():
     cfg = inputs.CFG3_NULL.scaled(150, 91)          # odd ray count: the last thread has an empty second slot
     ref = None
     try:
-        for shape in [(0, 0), (128, 3), (256, 2), (128, 8), (128, 6)]:
+        for shape in [(0, 0), (128, 3), (128, 4), (128, 8), (128, 6)]:
             gray2.set_launch(gray2.F32, *shape)
             _, g, stats = run_gpu_image(cfg, prec=gray2.F32)
             cur = (g.q.clone(), g.nsteps.clone(), g.status.clone(), g.lam.clone(), stats)
