@@ -85,6 +85,7 @@ def lib():
         _lib.oracle_rk4_step_coordtime.argtypes = [d, p, d]
         _lib.oracle_trajectory_coordtime.argtypes = [d, p, d, C.c_int64, C.c_int64, p]
         _lib.oracle_integrate_coordtime.argtypes = [p, C.c_uint64, d, p, p]
+        _lib.oracle_integrate_diagnostics.argtypes = [p, C.c_uint64, d, p, p, p]
         _lib.oracle_num_threads.restype = C.c_int
     return _lib
 
@@ -187,6 +188,20 @@ def integrate_coordtime(st: State, t_end, sc: _StepControl, n=None) -> dict:
     if rc:
         raise ValueError("oracle_integrate_coordtime: invalid arguments")
     return {k: int(getattr(stats, k)) for k, _ in _Stats._fields_}
+
+
+def integrate_diagnostics(st: State, lambda_end, sc: _StepControl, n=None):
+    """Integrate and accumulate the paper's convergence diagnostics.  Returns (stats, diag) with
+    diag = dict(max_abs_u2, cos_peak, dphi_cycle, t_zmax1, t_zmax2), each (n,) float64 (NaN = never)."""
+    n = st.n if n is None else n
+    out = np.empty((5, n), dtype=np.float64)
+    cs = st._c()
+    stats = _Stats()
+    rc = lib().oracle_integrate_diagnostics(C.byref(cs), n, float(lambda_end), C.byref(sc), _ptr(out), C.byref(stats))
+    if rc:
+        raise ValueError("oracle_integrate_diagnostics: invalid arguments")
+    names = ("max_abs_u2", "cos_peak", "dphi_cycle", "t_zmax1", "t_zmax2")
+    return {k: int(getattr(stats, k)) for k, _ in _Stats._fields_}, dict(zip(names, out))
 
 
 def invariants(st: State):

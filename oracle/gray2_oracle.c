@@ -11,6 +11,7 @@
  * circular-orbit period, ISCO, epicyclic frequency, Bardeen shadow, Carter radial potential,
  * independent Boyer-Lindquist integration.  No function is "parity unpinned".
  */
+#define _GNU_SOURCE
 #include "gray2_oracle.h"
 #include <math.h>
 #include <stddef.h>
@@ -459,6 +460,114 @@ int oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
       s->q[4][k] = 1.0;
       s->status[k] = st; s->nsteps[k] = ns;
     }
+    steps += (uint64_t)(ns - ns0);
+    nc += (st == ORACLE_CAPTURED); ne += (st == ORACLE_ESCAPED); nm += (st == ORACLE_MAXSTEPS);
+    ni += (st == ORACLE_INVALID);  na += (st == ORACLE_ACTIVE);
+  }
+  if (stats) {
+    stats->steps = steps; stats->n_captured = nc; stats->n_escaped = ne;
+    stats->n_maxsteps = nm; stats->n_invalid = ni; stats->n_active = na;
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Diagnostics of the paper's convergence experiments, accumulated over the samples k = 0,1,2,...
+ * (the states at the step boundaries of the driver loop above, the initial state included):
+ *   max_abs_u2  max_k | g u u + mu^2 |                          PAPER.md:217, :231 (Fig. 4-5)
+ *   cos_peak    first local maximum of c_k = |z_k| / r_k, refined by the quadratic through the three
+ *               samples around it: c_i - (c_{i+1}-c_{i-1})^2 / (8 (c_{i-1} - 2 c_i + c_{i+1}))
+ *                                                                PAPER.md:247 (Fig. 6-7)
+ *   dphi_cycle  unfolded KS azimuth phi = atan2(y,x) - atan2(a,r) advanced up to the first upward zero
+ *               of z (z_k < 0 <= z_{k+1}), located by linear interpolation, minus phi_0
+ *                                                                PAPER.md:249 (Fig. 8)
+ *   t_zmax1,2   KS times of the first two maxima of z, i.e. downward zeros of u^z (u^z_k > 0 >= u^z_{k+1}),
+ *               linear interpolation in t                        PAPER.md:263 (Fig. 9)
+ * Quantities that never occur are NaN.  out: 5 arrays of n doubles.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+  double u2max, cprev2, cprev1, peak, phi0, phiprev, phiunf, zprev, uzprev, tprev, dphi, tz[2];
+  int64_t k;
+  int have_peak, have_dphi, ntz;
+} diag_acc;
+
+static double wrap_pi(double d)
+{
+  while (d > M_PI) d -= 2.0 * M_PI;
+  while (d <= -M_PI) d += 2.0 * M_PI;
+  return d;
+}
+
+static void diag_sample(diag_acc *D, double a, int32_t kind, const double y[8])
+{
+  double inv[4];
+  oracle_invariants_one(a, kind, y, inv);
+  double u2 = fabs(inv[3] + (kind == ORACLE_TIMELIKE ? 1.0 : 0.0));
+  double r = oracle_ks_r(a, y[1], y[2], y[3]);
+  double c = fabs(y[3]) / r;
+  double phi = atan2(y[2], y[1]) - atan2(a, r);
+  if (D->k == 0) {
+    D->u2max = u2; D->phi0 = phi; D->phiunf = phi;
+  } else {
+    if (u2 > D->u2max) D->u2max = u2;
+    double phiunf = D->phiunf + wrap_pi(phi - D->phiprev);
+    if (D->k >= 2 && !D->have_peak && D->cprev1 >= D->cprev2 && D->cprev1 > c) {
+      double y0 = D->cprev2, y1 = D->cprev1, y2 = c;
+      D->peak = y1 - (y2 - y0) * (y2 - y0) / (8.0 * (y0 - 2.0 * y1 + y2));
+      D->have_peak = 1;
+    }
+    if (!D->have_dphi && D->k >= 2 && D->zprev < 0.0 && y[3] >= 0.0) {
+      double w = -D->zprev / (y[3] - D->zprev);
+      D->dphi = D->phiunf + w * (phiunf - D->phiunf) - D->phi0;
+      D->have_dphi = 1;
+    }
+    if (D->ntz < 2 && D->uzprev > 0.0 && y[7] <= 0.0) {
+      D->tz[D->ntz] = D->tprev + (y[0] - D->tprev) * D->uzprev / (D->uzprev - y[7]);
+      D->ntz += 1;
+    }
+    D->phiunf = phiunf;
+  }
+  D->cprev2 = D->cprev1; D->cprev1 = c;
+  D->phiprev = phi; D->zprev = y[3]; D->uzprev = y[7]; D->tprev = y[0];
+  D->k += 1;
+}
+
+int oracle_integrate_diagnostics(oracle_state *s, uint64_t n, double lambda_end,
+                                 const oracle_step_control *sc, double *out5n, oracle_stats *stats)
+{
+  if (!s || !sc || !out5n || n == 0 || n > s->n) return 1;
+  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return 1;
+  if (sc->dir != 1 && sc->dir != -1) return 1;
+  uint64_t steps = 0, nc = 0, ne = 0, nm = 0, ni = 0, na = 0;
+  const double a = s->a_eff, r_plus = 1.0 + sqrt(1.0 - a * a), dir = (double)sc->dir;
+#pragma omp parallel for schedule(dynamic, 4) reduction(+ : steps, nc, ne, nm, ni, na)
+  for (int64_t k = 0; k < (int64_t)n; ++k) {
+    double y[8];
+    for (int m = 0; m < 8; ++m) y[m] = s->q[m][k];
+    int32_t st = s->status[k], ns = s->nsteps[k], ns0 = ns;
+    double lam = s->lambda[k];
+    diag_acc D;
+    memset(&D, 0, sizeof D);
+    D.peak = D.dphi = D.tz[0] = D.tz[1] = NAN;
+    while (st == ORACLE_ACTIVE) {
+      double r = oracle_ks_r(a, y[1], y[2], y[3]);
+      if (!isfinite(r) || !all_finite(y)) { st = ORACLE_INVALID; break; }
+      diag_sample(&D, a, s->kind, y);
+      if (r < sc->capture_factor * r_plus) { st = ORACLE_CAPTURED; break; }
+      if (r > sc->r_escape) { st = ORACLE_ESCAPED; break; }
+      if (ns >= sc->max_steps) { st = ORACLE_MAXSTEPS; break; }
+      if (dir * (lambda_end - lam) <= 0.0) break;
+      double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
+      if (fabs(h) > fabs(lambda_end - lam)) h = lambda_end - lam;
+      oracle_rk4_step(a, y, h);
+      lam += h;
+      ns += 1;
+    }
+    for (int m = 0; m < 8; ++m) s->q[m][k] = y[m];
+    s->status[k] = st; s->nsteps[k] = ns; s->lambda[k] = lam;
+    out5n[0 * n + k] = D.k ? D.u2max : NAN;
+    out5n[1 * n + k] = D.peak; out5n[2 * n + k] = D.dphi;
+    out5n[3 * n + k] = D.tz[0]; out5n[4 * n + k] = D.tz[1];
     steps += (uint64_t)(ns - ns0);
     nc += (st == ORACLE_CAPTURED); ne += (st == ORACLE_ESCAPED); nm += (st == ORACLE_MAXSTEPS);
     ni += (st == ORACLE_INVALID);  na += (st == ORACLE_ACTIVE);

@@ -83,6 +83,12 @@ void   oracle_trajectory_coordtime(double a, const double y0[7], double h, int64
 int    oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
                                   const oracle_step_control *sc, oracle_stats *stats);
 
+/* ---- diagnostics of the paper's convergence experiments (section 3; Fig. 4-9), see gray2_oracle.c ----
+   out5n: 5 arrays of n doubles: max|u.u + mu^2|, first fitted peak of |cos theta|, Delta phi of the first
+   complete polar cycle, times of the first two maxima of z.  NaN where the event never occurs. */
+int    oracle_integrate_diagnostics(oracle_state *s, uint64_t n, double lambda_end,
+                                    const oracle_step_control *sc, double *out5n, oracle_stats *stats);
+
 /* ---- independent Boyer-Lindquist integrator (self-check only; eq. 1) ---- */
 void   oracle_bl_metric(double a, const double X[4], double g[16]);                 /* X = t,r,theta,phi  */
 void   oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4]);
