@@ -114,6 +114,27 @@ int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_s
 int gray2_integrate_coordtime(gray2_state *s, uint64_t n, double t_end, const gray2_step_control *sc,
                               int32_t prec, gray2_stats *device_stats, void *cuda_stream);
 
+/* Diagnostics of the paper's convergence experiments (section 3), accumulated over the
+ * samples k = 0, 1, 2, ... = the states at the step boundaries of this call, the initial state included.
+ * Five DEVICE arrays of n doubles, always evaluated in double; NaN where the event never occurs:
+ *   max_abs_u2  max_k |g u u + mu^2|, mu^2 nominal from s->kind                     (Fig. 4-5)
+ *   cos_peak    first local maximum of c_k = |z_k|/r_k refined by the quadratic through the three samples
+ *               around it: c_i - (c_{i+1}-c_{i-1})^2 / (8 (c_{i-1} - 2 c_i + c_{i+1}))  (Fig. 6-7)
+ *   dphi_cycle  unfolded KS azimuth phi = atan2(y,x) - atan2(a,r) at the first upward zero of z
+ *               (z_k < 0 <= z_{k+1}, linear interpolation) minus phi_0                  (Fig. 8)
+ *   t_zmax1,2   KS times of the first two maxima of z: downward zeros of u^z, linear interpolation in t
+ *                                                                                       (Fig. 9) */
+typedef struct {
+  double *max_abs_u2, *cos_peak, *dphi_cycle, *t_zmax1, *t_zmax2;
+} gray2_diagnostics;
+
+/* gray2_integrate (affine form, same step and stopping rule, same final state bit for bit) plus the
+ * diagnostics above.  One thread per geodesic: meant for the convergence studies (thousands of orbits),
+ * not for images.  The accumulators start afresh at every call. */
+int gray2_integrate_diagnostics(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                                int32_t prec, const gray2_diagnostics *diag, gray2_stats *device_stats,
+                                void *cuda_stream);
+
 /* Constants of the RUN geodesic, always evaluated in double from the stored state (DESIGN R8):
  *   norm = g_ab u^a u^b ;  E = -u_t ;  L_z = x u_y - y u_x ;
  *   Q = u_theta^2 + cos^2(theta) [ a^2 (mu^2 - E^2) + L_z^2 / sin^2(theta) ], mu^2 nominal from s->kind.

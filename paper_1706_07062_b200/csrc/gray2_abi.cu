@@ -197,6 +197,41 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, cons
 
 }  // namespace
 
+namespace {
+
+template <typename T>
+int diag_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                     const gray2_diagnostics *d, gray2_stats *device_stats, cudaStream_t st) {
+  const double a = s->a_eff;
+  gray2::StepParams<T> p;
+  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a);
+  p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
+  p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
+  p.r_escape = (T)sc->r_escape;
+  p.r_escape_fin = p.r_escape;
+  p.lambda_end = lambda_end; p.dir = (double)sc->dir; p.mode = sc->mode; p.max_steps = sc->max_steps; p.clip = 1;
+  unsigned slot = g_queue_next.fetch_add(1) % kQueueSlots;
+  unsigned long long *steps = g_queue + 8 * slot + 1;
+  CUDA_TRY(cudaMemsetAsync(steps, 0, sizeof(unsigned long long), st));
+  gray2::DiagView out{d->max_abs_u2, d->cos_peak, d->dphi_cycle, d->t_zmax1, d->t_zmax2};
+  double mu2 = s->kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
+  unsigned grid = (unsigned)((n + 63) / 64);
+  if (sc->mode == 1) gray2::integrate_diag_kernel<T, 1><<<grid, 64, 0, st>>>(view_of<T>(s), n, p, mu2, out, steps);
+  else gray2::integrate_diag_kernel<T, 0><<<grid, 64, 0, st>>>(view_of<T>(s), n, p, mu2, out, steps);
+  CUDA_TRY(cudaGetLastError());
+  if (device_stats) {
+    CUDA_TRY(cudaMemsetAsync(device_stats, 0, sizeof(gray2_stats), st));
+    CUDA_TRY(cudaMemcpyAsync(&device_stats->steps, steps, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st));
+    unsigned g2 = (unsigned)((n + 255) / 256);
+    if (g2 > (unsigned)(g_num_sms * 8)) g2 = (unsigned)(g_num_sms * 8);
+    gray2::count_status_kernel<<<g2, 256, 0, st>>>(s->status, n, device_stats);
+    CUDA_TRY(cudaGetLastError());
+  }
+  return GRAY2_OK;
+}
+
+}  // namespace
+
 // ---- the exported calls ------------------------------------------------------------------------------
 extern "C" {
 
@@ -288,6 +323,31 @@ int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_s
 int gray2_integrate_coordtime(gray2_state *s, uint64_t n, double t_end, const gray2_step_control *sc,
                               int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
   return integrate_common(1, "gray2_integrate_coordtime", s, n, t_end, sc, prec, device_stats, cuda_stream);
+}
+
+int gray2_integrate_diagnostics(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
+                                int32_t prec, const gray2_diagnostics *diag, gray2_stats *device_stats,
+                                void *cuda_stream) {
+  const char *who = "gray2_integrate_diagnostics";
+  int rc = check_state(s, who);
+  if (rc) return rc;
+  if (!sc || !diag) return fail(GRAY2_EINVAL, "%s: step control or diagnostics is NULL", who);
+  if (!diag->max_abs_u2 || !diag->cos_peak || !diag->dphi_cycle || !diag->t_zmax1 || !diag->t_zmax2)
+    return fail(GRAY2_EINVAL, "%s: a diagnostics array is NULL", who);
+  if (n == 0) return fail(GRAY2_EINVAL, "%s: n == 0", who);
+  if (n > s->n) return fail(GRAY2_ESTATE, "%s: n exceeds s->n", who);
+  if (prec != s->prec) return fail(GRAY2_EINVAL, "%s: prec differs from s->prec", who);
+  if (sc->mode != 0 && sc->mode != 1) return fail(GRAY2_EINVAL, "%s: mode must be 0 or 1", who);
+  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return fail(GRAY2_EINVAL, "%s: step size must be > 0", who);
+  if (sc->dir != 1 && sc->dir != -1) return fail(GRAY2_EINVAL, "%s: dir must be +1 or -1", who);
+  if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(lambda_end) || sc->max_steps < 0)
+    return fail(GRAY2_EINVAL, "%s: bad capture_factor / r_escape / lambda_end / max_steps", who);
+  if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a_eff| must be <= 1", who);
+  rc = ensure_scratch();
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  return prec == GRAY2_F64 ? diag_impl<double>(s, n, lambda_end, sc, diag, device_stats, st)
+                           : diag_impl<float>(s, n, lambda_end, sc, diag, device_stats, st);
 }
 
 int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm,

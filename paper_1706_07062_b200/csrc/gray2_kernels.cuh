@@ -308,6 +308,97 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
   if (lane == 0 && my_steps) atomicAdd(steps_out, my_steps);
 }
 
+// ---- integration with the paper's convergence diagnostics (section 3, Fig. 4-9) ----------------------
+// One thread per geodesic (these runs are small: thousands of orbits x a few step sizes).  The samples are
+// the states at the step boundaries, the initial state included; see gray2_diagnostics in gray2.h.
+struct DiagView {
+  double *max_abs_u2, *cos_peak, *dphi_cycle, *t_zmax1, *t_zmax2;
+};
+
+__device__ __forceinline__ double wrap_pi(double d) {
+  const double pi = 3.14159265358979323846;
+  while (d > pi) d -= 2.0 * pi;
+  while (d <= -pi) d += 2.0 * pi;
+  return d;
+}
+
+template <typename T, int MODE>
+__global__ void integrate_diag_kernel(StateView<T> s, uint64_t n, StepParams<T> p, double mu2, DiagView out,
+                                      unsigned long long *steps_out) {
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  const double nan = __longlong_as_double(0x7ff8000000000000LL);
+  if (s.status[idx] != GRAY2_ACTIVE) {   // not touched: no samples, every diagnostic is NaN
+    out.max_abs_u2[idx] = nan; out.cos_peak[idx] = nan; out.dphi_cycle[idx] = nan;
+    out.t_zmax1[idx] = nan; out.t_zmax2[idx] = nan;
+    return;
+  }
+  const SpinConst<T> k = p.k;
+  Ray<T> ray;
+  ray.t = s.q[0][idx]; ray.x = s.q[1][idx]; ray.y = s.q[2][idx]; ray.z = s.q[3][idx];
+  ray.u0 = s.q[4][idx]; ray.u1 = s.q[5][idx]; ray.u2 = s.q[6][idx]; ray.u3 = s.q[7][idx];
+  double lam = s.lambda[idx];
+  int32_t nst = s.nsteps[idx], nst0 = nst, st = GRAY2_ACTIVE;
+  // accumulators
+  double u2max = nan, c2 = 0.0, c1 = 0.0, peak = nan, phi0 = 0.0, phiprev = 0.0, phiunf = 0.0;
+  double zprev = 0.0, uzprev = 0.0, tprev = 0.0, dphi = nan, tz0 = nan, tz1 = nan;
+  long long ks = 0;
+  int ntz = 0;
+  bool have_peak = false, have_dphi = false;
+  for (;;) {
+    Geometry<T> g;
+    ks_geometry(k, ray.x, ray.y, ray.z, g);
+    T U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+    if (!(fastmath<T>::finite(g.r) && fastmath<T>::finite(U) && fastmath<T>::finite(ray.t))) { st = GRAY2_INVALID; break; }
+    {   // ---- sample k ----
+      double u0 = (double)ray.u0, u1 = (double)ray.u1, u2 = (double)ray.u2, u3 = (double)ray.u3;
+      double Ud = (double)U, fd = (double)g.f, r = (double)g.r, z = (double)ray.z, t = (double)ray.t;
+      double nrm = fabs(-u0 * u0 + u1 * u1 + u2 * u2 + u3 * u3 + fd * Ud * Ud + mu2);
+      double c = fabs(z) / r;
+      double phi = atan2((double)ray.y, (double)ray.x) - atan2((double)k.a, r);
+      if (ks == 0) {
+        u2max = nrm; phi0 = phi; phiunf = phi;
+      } else {
+        if (nrm > u2max) u2max = nrm;
+        double unf = phiunf + wrap_pi(phi - phiprev);
+        if (ks >= 2 && !have_peak && c1 >= c2 && c1 > c) {
+          peak = c1 - (c - c2) * (c - c2) / (8.0 * (c2 - 2.0 * c1 + c));
+          have_peak = true;
+        }
+        if (!have_dphi && ks >= 2 && zprev < 0.0 && z >= 0.0) {
+          double w = -zprev / (z - zprev);
+          dphi = phiunf + w * (unf - phiunf) - phi0;
+          have_dphi = true;
+        }
+        if (ntz < 2 && uzprev > 0.0 && u3 <= 0.0) {
+          double tt = tprev + (t - tprev) * uzprev / (uzprev - u3);
+          if (ntz == 0) tz0 = tt; else tz1 = tt;
+          ntz += 1;
+        }
+        phiunf = unf;
+      }
+      c2 = c1; c1 = c; phiprev = phi; zprev = z; uzprev = u3; tprev = t;
+      ks += 1;
+    }
+    if (g.r < p.r_capture) { st = GRAY2_CAPTURED; break; }
+    if (g.r > p.r_escape) { st = GRAY2_ESCAPED; break; }
+    if (nst >= p.max_steps) { st = GRAY2_MAXSTEPS; break; }
+    if (p.dir * (p.lambda_end - lam) <= 0.0) break;
+    T h = (MODE == 1) ? p.eta_or_h * g.r : p.eta_or_h;
+    double hd = (double)h, rem = p.lambda_end - lam;
+    if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
+    rk4_step(k, ray, g, h);
+    lam += hd;
+    nst += 1;
+  }
+  s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
+  s.q[4][idx] = ray.u0; s.q[5][idx] = ray.u1; s.q[6][idx] = ray.u2; s.q[7][idx] = ray.u3;
+  s.lambda[idx] = lam; s.status[idx] = st; s.nsteps[idx] = nst;
+  out.max_abs_u2[idx] = u2max; out.cos_peak[idx] = peak; out.dphi_cycle[idx] = dphi;
+  out.t_zmax1[idx] = tz0; out.t_zmax2[idx] = tz1;
+  if (nst > nst0) atomicAdd(steps_out, (unsigned long long)(nst - nst0));
+}
+
 // ---- invariants (always double) ------------------------------------------------------------------
 template <typename T>
 __global__ void invariants_kernel(StateView<T> s, uint64_t n, double a, double mu2, double *__restrict__ E,

@@ -72,6 +72,8 @@ def load_library():
     lib.gray2_flops_per_step_coordtime.argtypes = [i32]
     lib.gray2_flops_per_step_coordtime.restype = C.c_int
     lib.gray2_invariants.argtypes = [p, u64, p, p, p, p, p]
+    lib.gray2_integrate_diagnostics.argtypes = [p, u64, d, p, i32, p, p, p]
+    lib.gray2_integrate_diagnostics.restype = C.c_int
     lib.gray2_rhs.argtypes = [i32, d, u64, p, p, p, p]
     lib.gray2_set_launch.argtypes = [i32, i32, i32]
     lib.gray2_fma_probe.argtypes = [i32, i32, i32, i32, i32, p, p]
@@ -185,6 +187,23 @@ def integrate_coordtime(st: State, t_end, sc: StepControl, n=None, stats: torch.
     _check(load_library().gray2_integrate_coordtime(C.byref(cs), st.n if n is None else n, float(t_end),
                                                     C.byref(sc), st.prec, sp, _stream_ptr(stream)))
     return stats
+
+
+DIAG_FIELDS = ("max_abs_u2", "cos_peak", "dphi_cycle", "t_zmax1", "t_zmax2")
+
+
+def integrate_diagnostics(st: State, lambda_end, sc: StepControl, n=None, stats: torch.Tensor | None = None,
+                          stream=None) -> dict:
+    """gray2_integrate_diagnostics: integrate and return the paper's convergence diagnostics as a dict of
+    five cuda float64 tensors (see gray2_diagnostics in gray2.h)."""
+    n = st.n if n is None else n
+    out = torch.empty((5, n), dtype=torch.float64, device=st.q.device)
+    ptrs = (C.c_void_p * 5)(*[out[k].data_ptr() for k in range(5)])
+    cs = st._c()
+    sp = C.c_void_p(stats.data_ptr()) if stats is not None else C.c_void_p(0)
+    _check(load_library().gray2_integrate_diagnostics(C.byref(cs), n, float(lambda_end), C.byref(sc), st.prec,
+                                                      C.byref(ptrs), sp, _stream_ptr(stream)))
+    return dict(zip(DIAG_FIELDS, out))
 
 
 def new_stats(device="cuda") -> torch.Tensor:

@@ -1,0 +1,127 @@
+"""GPU parity of gray2_integrate_diagnostics (the paper's convergence diagnostics, section 3) against the
+oracle, and a batch-scale rerun of the paper's convergence study (Fig. 5, 7, 8) on the GPU."""
+import numpy as np
+import pytest
+import torch
+
+import closed_forms as cf
+import oracle
+from conftest import load_table1
+from gpu_helpers import INF, TOL_STATE_F64, sc_pair, state_rel_error, to_oracle_state
+from paper_1706_07062_b200 import gray2, inputs
+
+pytestmark = pytest.mark.gpu
+ROWS = load_table1()
+
+
+def table1_xu8():
+    return np.array([cf.spherical_photon_state(1.0, r["r"])[0] for r in ROWS])
+
+
+def run_pair(a, xu8, kind, lam_end, **kw):
+    gsc, osc = sc_pair(**kw)
+    g = gray2.init_timelike(a, xu8)
+    g.kind = kind
+    o = oracle.init_timelike(a, xu8)
+    o.kind = kind
+    stats = gray2.new_stats()
+    gd = gray2.integrate_diagnostics(g, lam_end, gsc, stats=stats)
+    ostats, od = oracle.integrate_diagnostics(o, lam_end, osc)
+    return g, o, {k: v.cpu().numpy() for k, v in gd.items()}, od, gray2.stats_dict(stats), ostats
+
+
+def close(gv, ov, atol, rtol=0.0):
+    both_nan = np.isnan(gv) & np.isnan(ov)
+    return np.all(both_nan | (np.abs(gv - ov) <= atol + rtol * np.abs(ov)))
+
+
+def test_table1_diagnostics_match_oracle_and_paper():
+    xu8 = np.repeat(table1_xu8(), 11, axis=0)            # 66 orbits: more than one block of 64, ragged
+    g, o, gd, od, gs, os_ = run_pair(1.0, xu8, gray2.NULL, 24.0, mode=0, h_fixed=1.0 / 128, max_steps=10 ** 7)
+    assert gs == os_ and gs["n_active"] == 66
+    gst = to_oracle_state(g)
+    # unstable orbits: the 1e-16 rounding difference of the two sides has grown by e^(kappa lambda)
+    # at lambda = 24, so the final states agree to 1e-6 only; the diagnostics below are early-time quantities
+    assert np.array_equal(gst.nsteps, o.nsteps) and state_rel_error(gst.q, o.q, 1.0).max() < 1e-6
+    assert close(gd["cos_peak"], od["cos_peak"], 1e-12) and close(gd["dphi_cycle"], od["dphi_cycle"], 1e-10)
+    assert close(gd["t_zmax1"], od["t_zmax1"], 1e-9) and close(gd["t_zmax2"], od["t_zmax2"], 1e-9)
+    assert close(gd["max_abs_u2"], od["max_abs_u2"], 1e-15, rtol=1e-3)
+    for k, row in enumerate(ROWS):                        # and the paper's printed values
+        assert abs(gd["cos_peak"][11 * k] - row["maxcos"]) < 6e-5
+        d = gd["dphi_cycle"][11 * k]
+        if row["label"] == "C":
+            d = (d - row["dphi"] + np.pi) % (2 * np.pi) - np.pi + row["dphi"]
+        assert abs(d - row["dphi"]) < 6e-5
+
+
+def test_same_final_state_as_gray2_integrate():
+    xu8, _ = inputs.cfg4_ensemble(300)
+    gsc, _ = sc_pair(mode=0, h_fixed=0.5, max_steps=900)
+    a_ = gray2.init_timelike(0.7, xu8)
+    b_ = gray2.init_timelike(0.7, xu8)
+    gray2.integrate(a_, INF, gsc)
+    d = gray2.integrate_diagnostics(b_, INF, gsc)
+    assert torch.equal(a_.q, b_.q) and torch.equal(a_.nsteps, b_.nsteps) and torch.equal(a_.status, b_.status)
+    assert torch.equal(a_.lam, b_.lam)
+    assert torch.isfinite(d["max_abs_u2"]).all() and (d["max_abs_u2"] < 1e-3).all() and d["max_abs_u2"].median() < 1e-9
+
+
+def test_epicyclic_frequency_batch_on_gpu():
+    # PAPER.md:263-269 (Fig. 9) at batch scale: 64 radii, a = 1, v_z = 1e-12
+    a = 1.0
+    radii = np.linspace(1.3, 12.0, 64)
+    xu8 = np.array([cf.circular_orbit_state(a, r, +1, vz=1e-12) for r in radii])
+    expect = np.array([cf.vertical_epicyclic(a, r, +1) for r in radii])
+    ut = np.array([cf.circular_orbit(a, r, +1)[3] for r in radii])
+    h = float(np.min(2 * np.pi / expect / ut) / 1024.0)
+    nsteps = int(np.max(2 * np.pi / expect / ut) / h * 2.4)
+    g = gray2.init_timelike(a, xu8)
+    d = gray2.integrate_diagnostics(g, INF, gray2.step_control(mode=0, h_fixed=h, max_steps=nsteps))
+    measured = 2 * np.pi / (d["t_zmax2"] - d["t_zmax1"]).cpu().numpy()
+    assert np.isfinite(measured).all() and np.abs(measured / expect - 1.0).max() < 5e-6   # RK4 truncation at r = 1.3
+    # sampled against the oracle
+    idx = [0, 17, 40, 63]
+    o = oracle.init_timelike(a, xu8[idx])
+    _, od = oracle.integrate_diagnostics(o, INF, oracle.step_control(mode=0, h_fixed=h, max_steps=nsteps))
+    assert np.abs(d["t_zmax1"].cpu().numpy()[idx] - od["t_zmax1"]).max() < 1e-7
+    assert np.abs(d["t_zmax2"].cpu().numpy()[idx] - od["t_zmax2"]).max() < 1e-7
+
+
+def test_convergence_study_of_the_paper_on_the_gpu():
+    """Fig. 5, 7, 8 in one launch: the six Table 1 orbits x five step sizes cannot share a launch (the step
+    is a launch parameter), so five launches; errors must fall 16x per halving."""
+    xu8 = table1_xu8()
+    exact_peak = np.array([cf.max_abs_costheta(1.0, *cf.teo_phi_q(1.0, r["r"])) for r in ROWS])
+    u2, pk, dp = [], [], []
+    for n in (16, 32, 64, 128, 256):
+        g = gray2.init_timelike(1.0, xu8)
+        g.kind = gray2.NULL
+        d = gray2.integrate_diagnostics(g, 6.0 if n < 256 else 24.0, gray2.step_control(mode=0, h_fixed=1.0 / n, max_steps=10 ** 7))
+        u2.append(d["max_abs_u2"].cpu().numpy())
+        pk.append(np.abs(d["cos_peak"].cpu().numpy() - exact_peak))
+        dp.append(d["dphi_cycle"].cpu().numpy())
+    u2, pk = np.array(u2), np.array(pk)
+    r_u2 = u2[:3] / u2[1:4]
+    assert ((r_u2 > 8) & (r_u2 < 30)).all(), r_u2
+    sel = [0, 1, 3]                                       # A, B, D: peaks far from |cos| = 1
+    r_pk = pk[:3][:, sel] / pk[1:4][:, sel]
+    assert ((r_pk > 8) & (r_pk < 32)).all(), r_pk
+
+
+def test_fp32_diagnostics_and_edges():
+    xu8 = table1_xu8()
+    g = gray2.init_timelike(1.0, xu8, prec=gray2.F32)
+    g.kind = gray2.NULL
+    d = gray2.integrate_diagnostics(g, 10.0, gray2.step_control(mode=0, h_fixed=1.0 / 64, max_steps=10 ** 6))
+    pk = d["cos_peak"].cpu().numpy()
+    assert np.abs(pk - np.array([r["maxcos"] for r in ROWS])).max() < 2e-3
+    # INVALID input: NaN diagnostics, zero steps; non-ACTIVE rays are left alone
+    x = xu8.copy()
+    x[1, 5] = np.nan
+    g2 = gray2.init_timelike(1.0, x)
+    g2.status[2] = gray2.ESCAPED
+    stats = gray2.new_stats()
+    d2 = gray2.integrate_diagnostics(g2, 3.0, gray2.step_control(mode=0, h_fixed=0.1, max_steps=1000), stats=stats)
+    sd = gray2.stats_dict(stats)
+    assert g2.status[1].item() == gray2.INVALID and g2.nsteps[1].item() == 0 and torch.isnan(d2["max_abs_u2"][1])
+    assert sd["n_invalid"] == 1 and sd["n_escaped"] == 1 and sd["n_active"] == 4 and sd["steps"] == 4 * 30
