@@ -35,6 +35,11 @@ INF = float("inf")
 # (128 FP32 lanes) x 2 flops per FMA x 1.965 GHz (clocks.max.sm of this pool, MEASURED_PEAKS.json).
 FP_LANES = {"f64": 64, "f32": 128}
 
+# DRAM traffic of the dominant kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch, from the
+# `ncu --set full` captures summarised in profiles/r01_ncu_integrate_f{64,32}_v3.txt (cfg3, affine form).
+# Algorithmic state traffic is 2 x 80 B (FP64) or 2 x 48 B (FP32) per ray.
+NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83903744 + 31966464, ("cfg3", "f32", "affine"): 50362880 + 1761536}
+
 
 def nominal_peak_tflops(dtype: str, n_sms: int, sm_max_mhz: float) -> float:
     return n_sms * FP_LANES[dtype] * 2.0 * sm_max_mhz * 1e6 / 1e12
@@ -163,7 +168,6 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------
 
 def run_gpu(args):
-    import numpy as np
     import torch
     import torch.distributed as dist
 
@@ -315,7 +319,9 @@ def run_gpu(args):
             "roofline": {"bound": "alu", "kernel": ("integrate_kernel<double%s>" if prec == gray2.F64 else "integrate_kernel_f32x2<%s>") % (
                              ", coordinate time" if coord else ("" if prec == gray2.F64 else "affine")),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": None, "flops_per_rk4_step": flops_per_step,
+                         "traffic": NCU_DRAM_BYTES.get((args.workload, args.dtype, args.form)),
+                         "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_integrate_*_v3.txt)",
+                         "flops_per_rk4_step": flops_per_step,
                          "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,
                          "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (n_sms, FP_LANES[args.dtype], sm_max_mhz),
                          "fma_probe_tflops": fma_probe_tflops, "frac_of_fma_probe": achieved / fma_probe_tflops,

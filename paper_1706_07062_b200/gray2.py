@@ -10,7 +10,6 @@ Function names match the C entry points: ``init_null``, ``init_timelike``, ``int
 from __future__ import annotations
 
 import ctypes as C
-import math
 import os
 from dataclasses import dataclass
 

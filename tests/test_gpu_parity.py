@@ -59,11 +59,10 @@ def test_init_timelike_matches_oracle():
         o = oracle.init_timelike(0.7, x, renormalise_ut=renorm)
         assert np.max(np.abs(g.q.cpu().numpy() - o.q) / np.maximum(np.abs(o.q), 1.0)) < 1e-14
         assert (g.a_eff, g.kind, g.reversed) == (0.7, gray2.TIMELIKE, 0)
-    if True:
-        gi = gpu_invariants_np(gray2.init_timelike(0.7, xu8))
-        oi = oracle.invariants(oracle.init_timelike(0.7, xu8))
-        for a_, b_ in zip(gi, oi):
-            assert np.max(np.abs(a_ - b_) / np.maximum(np.abs(b_), 1.0)) < 1e-13
+    gi = gpu_invariants_np(gray2.init_timelike(0.7, xu8))
+    oi = oracle.invariants(oracle.init_timelike(0.7, xu8))
+    for a_, b_ in zip(gi, oi):
+        assert np.max(np.abs(a_ - b_) / np.maximum(np.abs(b_), 1.0)) < 1e-13
 
 
 # ---- whole path on image configs ------------------------------------------------------------------
