@@ -158,3 +158,27 @@ def test_fp32_against_oracle(cfg):
     # bulk of the rays within the stated tolerance; the few strongly lensed ones amplify FP32 rounding
     assert np.quantile(err, 0.90) < TOL_STATE_F32, np.quantile(err, [0.5, 0.9, 0.99, 1.0])
     assert np.median(err) < 0.2 * TOL_STATE_F32
+
+
+@pytest.mark.parametrize("a,inc_deg", [(1.0, 80.0), (0.9375, 0.0), (-0.99, 180.0), (0.0, 0.0)],
+                         ids=["extremal-spin", "face-on", "face-on-from-below-retrograde", "schwarzschild-pole"])
+def test_degenerate_geometries(a, inc_deg):
+    """Extremal spin, and the face-on view in which the rays run along the spin axis through the poles
+    (the case that crashes Boyer-Lindquist integrators): no special handling exists or is
+    needed.  The band machinery needs sin(i) != 0 and |a| < 1, so agreement is asserted on every ray whose
+    step count equals the oracle's, and those must be all but a handful of near-critical rays."""
+    cfg = inputs.NullImageConfig("t", a, 1000.0, inc_deg, 9.0, 64, 48)
+    g0, g, gstats = run_gpu_image(cfg)
+    o0, o, ostats = run_oracle_image(cfg)
+    gst = to_oracle_state(g)
+    same = (gst.nsteps == o.nsteps) & (gst.status == o.status)
+    assert same.mean() > 0.995, same.mean()
+    assert (gst.status == o.status).mean() > 0.999
+    assert state_rel_error(gst.q[:, same], o.q[:, same], o.a_eff).max() < TOL_STATE_F64
+    assert gstats["n_invalid"] == 0 and gstats["n_active"] == 0 and gstats["n_maxsteps"] == ostats["n_maxsteps"]
+    if inc_deg in (0.0, 180.0):
+        # axisymmetry about the line of sight: the captured region is a disc centred on the image centre
+        alpha, beta = ih.pixel_grid(cfg)
+        b = np.hypot(alpha, beta)
+        cap = gst.status == gray2.CAPTURED
+        assert b[cap].max() < b[~cap].min() + 2 * cfg.fov / 48
