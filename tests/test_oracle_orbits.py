@@ -247,3 +247,32 @@ def test_renormalise_ut_gives_unit_norm():
     assert np.abs(oracle.invariants(st)[3] + 1.0).max() < 1e-13 and (st.q[4] > 0).all()
     raw = oracle.init_timelike(0.8, xu8, renormalise_ut=False)
     assert np.array_equal(raw.q[4], xu8[:, 4])
+
+
+# ---- equatorial circular photon orbits, eq. (19)-(20) ----------------------------
+
+@pytest.mark.parametrize("a", [0.5, 0.9])
+def test_circular_photon_orbit_radii_of_eq19_eq20(a):
+    rp, rr = cf.r_photon_prograde(a), cf.r_photon_retrograde(a)
+    assert 1.0 <= rp <= 3.0 <= rr <= 4.0                               # the inequality below eq. (20)
+    for r0, sign in ((rp, +1), (rr, -1)):
+        phi, q = cf.teo_phi_q(a, r0)
+        assert abs(q) < 1e-9 and np.sign(phi) == sign                   # equatorial (Q = 0), pro-/retrograde
+        y0, _, _ = cf.spherical_photon_state(a, r0)
+        y0[7] = 0.0                                                     # Q = 0 up to rounding: stay in the plane
+        traj = oracle.trajectory(a, y0, 1.0 / 512, 512 * 6, stride=64)
+        assert np.abs(radius(a, traj) - r0).max() < 1e-6                # circular (unstable: truncation error grows)
+        assert np.abs(traj[:, 3]).max() < 1e-12
+        ang = np.unwrap(np.arctan2(traj[:, 2], traj[:, 1]))
+        assert np.sign(ang[-1] - ang[0]) == sign
+        # a photon slightly outside r_r escapes, slightly inside r_p is captured (same constants of motion)
+    for r0, eps, expect in ((rr, +2e-3, oracle.ESCAPED), (rp, -2e-3, oracle.CAPTURED)):
+        y0, _, _ = cf.spherical_photon_state(a, r0)
+        y0[7] = 0.0
+        scale = (r0 + eps) / r0
+        y0[1] *= scale
+        y0[2] *= scale
+        st = oracle.init_timelike(a, y0[None, :])
+        st.kind = oracle.NULL
+        oracle.integrate(st, INF, oracle.step_control(mode=0, h_fixed=1.0 / 64, r_escape=40.0, max_steps=400000))
+        assert st.status[0] == expect
