@@ -252,25 +252,43 @@ def run_gpu(args):
     host_in.copy_(src.q.t())          # outside the timed region: the user's 8-vectors, resident in host memory
     a_eff = src.a_eff
     del src
-    host_q = torch.empty(st.q.shape, dtype=st.q.dtype).pin_memory()
-    host_lam = torch.empty(cfg.n, dtype=torch.float64).pin_memory()
-    host_status = torch.empty(cfg.n, dtype=torch.int32).pin_memory()
-    host_nsteps = torch.empty(cfg.n, dtype=torch.int32).pin_memory()
-    host_inv = torch.empty((4, cfg.n), dtype=torch.float64).pin_memory()
-    host_stats = torch.empty(6, dtype=torch.int64).pin_memory()
+    # The batch is cut into chunks that alternate between two streams, so that the H2D copy of one chunk
+    # and the D2H copy of another overlap the integration of a third (every call below is the public API).
+    # Each chunk has its own contiguous device state and pinned host result buffers, so every copy is a
+    # plain asynchronous memcpy.
+    n_chunks = max(1, args.e2e_chunks)
+    bounds = [(cfg.n * c // n_chunks, cfg.n * (c + 1) // n_chunks) for c in range(n_chunks)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    host_in_np = host_in.numpy()
+    parts, host_out, chunk_stats = [], [], []
+    for lo, hi in bounds:
+        m = hi - lo
+        parts.append(gray2.State.empty(m, prec))
+        chunk_stats.append(gray2.new_stats())
+        host_out.append(dict(q=torch.empty((8, m), dtype=st.q.dtype).pin_memory(),
+                             lam=torch.empty(m, dtype=torch.float64).pin_memory(),
+                             status=torch.empty(m, dtype=torch.int32).pin_memory(),
+                             nsteps=torch.empty(m, dtype=torch.int32).pin_memory(),
+                             inv=torch.empty((4, m), dtype=torch.float64).pin_memory(),
+                             stats=torch.empty(6, dtype=torch.int64).pin_memory()))
     h2d = host_in.numel() * 8
-    d2h = sum(t.numel() * t.element_size() for t in (host_q, host_lam, host_status, host_nsteps, host_inv, host_stats))
+    d2h = sum(t.numel() * t.element_size() for ho in host_out for t in ho.values())
 
     def e2e_step():
-        gray2.init_timelike(a_eff, host_in.numpy(), prec=prec, out=st)      # H2D inside (explicit 8-vectors)
-        st.kind, st.reversed = gray2.NULL, 1
-        integrate(st, INF, sc, stats=stats)
-        inv = gray2.invariants(st)
-        host_q.copy_(st.q, non_blocking=True); host_lam.copy_(st.lam, non_blocking=True)
-        host_status.copy_(st.status, non_blocking=True); host_nsteps.copy_(st.nsteps, non_blocking=True)
-        host_inv.copy_(torch.stack(inv), non_blocking=True); host_stats.copy_(stats, non_blocking=True)
+        for c, (lo, hi) in enumerate(bounds):
+            part, ho = parts[c], host_out[c]
+            with torch.cuda.stream(streams[c % 2]):
+                gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=part)   # H2D inside (explicit 8-vectors)
+                part.kind, part.reversed = gray2.NULL, 1
+                integrate(part, INF, sc, stats=chunk_stats[c])
+                inv = gray2.invariants(part)
+                ho["q"].copy_(part.q, non_blocking=True); ho["lam"].copy_(part.lam, non_blocking=True)
+                ho["status"].copy_(part.status, non_blocking=True); ho["nsteps"].copy_(part.nsteps, non_blocking=True)
+                for k in range(4):
+                    ho["inv"][k].copy_(inv[k], non_blocking=True)
+                ho["stats"].copy_(chunk_stats[c], non_blocking=True)
         torch.cuda.synchronize()
-        return int(host_stats[0])
+        return sum(int(ho["stats"][0]) for ho in host_out)
 
     e2e_step()
     e2e_n = max(1, min(args.steps, 3))
@@ -314,7 +332,8 @@ def run_gpu(args):
                        "parallelism": "independent image per GPU, no collective"},
             "clocks": clocks,
             "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "gray2_init_timelike(host 8-vectors) -> gray2_integrate -> gray2_invariants -> D2H of state, invariants, stats"},
+                    "api": "gray2_init_timelike(host 8-vectors) -> gray2_integrate -> gray2_invariants -> D2H of state, invariants, stats",
+                    "chunks": n_chunks, "streams": 2},
             "gpu_launches": 4 * args.steps,
             "roofline": {"bound": "alu", "kernel": ("integrate_kernel<double%s>" if prec == gray2.F64 else "integrate_kernel_f32x2<%s>") % (
                              ", coordinate time" if coord else ("" if prec == gray2.F64 else "affine")),
@@ -352,6 +371,7 @@ def main():
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--blocks", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-chunks", type=int, default=8, help="end-to-end leg: chunks pipelined over two streams")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
