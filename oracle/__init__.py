@@ -23,6 +23,7 @@ _LIB = os.path.join(_HERE, "liboracle_gray2.so")
 
 ACTIVE, CAPTURED, ESCAPED, MAXSTEPS, INVALID = 0, 1, 2, 3, 4
 NULL, TIMELIKE = 0, 1
+KS, BL = 0, 1
 
 
 def build(force: bool = False) -> str:
@@ -40,7 +41,7 @@ def build(force: bool = False) -> str:
 class _State(C.Structure):
     _fields_ = [("q", C.c_void_p * 8), ("lam", C.c_void_p), ("status", C.c_void_p),
                 ("nsteps", C.c_void_p), ("n", C.c_uint64), ("a_eff", C.c_double),
-                ("kind", C.c_int32), ("reversed", C.c_int32)]
+                ("kind", C.c_int32), ("reversed", C.c_int32), ("coords", C.c_int32)]
 
 
 class _StepControl(C.Structure):
@@ -76,6 +77,14 @@ def lib():
         _lib.oracle_trajectory.argtypes = [d, p, d, C.c_int64, C.c_int64, p]
         _lib.oracle_bl_metric.argtypes = [d, p, p]
         _lib.oracle_bl_accel.argtypes = [d, p, p, p]
+        _lib.oracle_bl_accel_fd.argtypes = [d, p, p, p]
+        _lib.oracle_bl_dmetric.argtypes = [d, p, p]
+        _lib.oracle_bl_dmetric_fd.argtypes = [d, p, p]
+        _lib.oracle_bl_rk4_step.argtypes = [d, p, d]
+        _lib.oracle_bl_invariants_one.argtypes = [d, C.c_int32, p, p]
+        _lib.oracle_bl_to_ks_one.argtypes = [d, p, p]
+        _lib.oracle_ks_to_bl_one.argtypes = [d, p, p]
+        _lib.oracle_convert.argtypes = [p, p, C.c_uint64, C.c_int32]
         _lib.oracle_bl_trajectory.argtypes = [d, p, d, C.c_int64, C.c_int64, p]
         _lib.oracle_init_null.argtypes = [p, d, d, d, d, d, C.c_int32, C.c_int32]
         _lib.oracle_init_timelike.argtypes = [p, d, p, C.c_uint64, C.c_int32]
@@ -104,13 +113,15 @@ def _vec(v, n):
 class State:
     """Host SoA state of n geodesics (same fields as gray2_state in include/gray2.h)."""
     n: int
-    q: np.ndarray = field(default=None)        # (8, n) float64 : t,x,y,z,u^t,u^x,u^y,u^z
+    q: np.ndarray = field(default=None)        # (8, n) float64 : t,x,y,z,u^t,u^x,u^y,u^z (KS) or
+                                               #                  t,r,theta,phi,u^t,u^r,u^theta,u^phi (BL)
     lam: np.ndarray = field(default=None)      # (n,) float64
     status: np.ndarray = field(default=None)   # (n,) int32
     nsteps: np.ndarray = field(default=None)   # (n,) int32
     a_eff: float = 0.0
     kind: int = NULL
     reversed: int = 0
+    coords: int = KS
 
     def __post_init__(self):
         if self.q is None:
@@ -130,14 +141,15 @@ class State:
         s.a_eff = self.a_eff
         s.kind = self.kind
         s.reversed = self.reversed
+        s.coords = self.coords
         return s
 
     def _back(self, s: _State):
-        self.a_eff, self.kind, self.reversed = s.a_eff, s.kind, s.reversed
+        self.a_eff, self.kind, self.reversed, self.coords = s.a_eff, s.kind, s.reversed, s.coords
 
     def copy(self) -> "State":
         return State(self.n, self.q.copy(), self.lam.copy(), self.status.copy(), self.nsteps.copy(),
-                     self.a_eff, self.kind, self.reversed)
+                     self.a_eff, self.kind, self.reversed, self.coords)
 
 
 def step_control(mode=1, h_fixed=0.0, eta=0.01, dir=1, capture_factor=1.01, r_escape=float("inf"),
@@ -312,6 +324,60 @@ def bl_accel(a, X, u):
     X, u = _vec(X, 4), _vec(u, 4)
     out = np.empty(4, dtype=np.float64)
     lib().oracle_bl_accel(a, _ptr(X), _ptr(u), _ptr(out))
+    return out
+
+
+def bl_accel_fd(a, X, u):
+    X, u = _vec(X, 4), _vec(u, 4)
+    out = np.empty(4, dtype=np.float64)
+    lib().oracle_bl_accel_fd(a, _ptr(X), _ptr(u), _ptr(out))
+    return out
+
+
+def bl_dmetric(a, X, fd=False):
+    """dg[c, a, b] = d_c g_ab of PAPER.md eq. (1); fd=True: 4th-order central differences of bl_metric."""
+    X = _vec(X, 4)
+    out = np.empty(64, dtype=np.float64)
+    (lib().oracle_bl_dmetric_fd if fd else lib().oracle_bl_dmetric)(a, _ptr(X), _ptr(out))
+    return out.reshape(4, 4, 4)
+
+
+def bl_rk4_step(a, y, h):
+    y = _vec(y, 8).copy()
+    lib().oracle_bl_rk4_step(a, _ptr(y), h)
+    return y
+
+
+def bl_invariants_one(a, kind, y):
+    y = _vec(y, 8)
+    out = np.empty(4, dtype=np.float64)
+    lib().oracle_bl_invariants_one(a, kind, _ptr(y), _ptr(out))
+    return out
+
+
+def bl_to_ks_one(a, y):
+    y = _vec(y, 8)
+    out = np.empty(8, dtype=np.float64)
+    lib().oracle_bl_to_ks_one(a, _ptr(y), _ptr(out))
+    return out
+
+
+def ks_to_bl_one(a, y):
+    y = _vec(y, 8)
+    out = np.empty(8, dtype=np.float64)
+    lib().oracle_ks_to_bl_one(a, _ptr(y), _ptr(out))
+    return out
+
+
+def convert(st: State, to_coords: int, n=None) -> State:
+    """A new State in the other coordinate system (KS <-> BL), same geodesics."""
+    n = st.n if n is None else n
+    out = State(st.n)
+    cs, cd = st._c(), out._c()
+    rc = lib().oracle_convert(C.byref(cs), C.byref(cd), n, to_coords)
+    if rc != 0:
+        raise ValueError("oracle_convert: bad arguments")
+    out._back(cd)
     return out
 
 

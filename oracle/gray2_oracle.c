@@ -249,7 +249,8 @@ int oracle_invariants(const oracle_state *s, uint64_t n, double *E, double *Lz, 
   for (int64_t k = 0; k < (int64_t)n; ++k) {
     double y[8], o[4];
     for (int m = 0; m < 8; ++m) y[m] = s->q[m][k];
-    oracle_invariants_one(s->a_eff, s->kind, y, o);
+    if (s->coords == ORACLE_BL) oracle_bl_invariants_one(s->a_eff, s->kind, y, o);
+    else oracle_invariants_one(s->a_eff, s->kind, y, o);
     E[k] = o[0]; Lz[k] = o[1]; Q[k] = o[2]; norm[k] = o[3];
   }
   return 0;
@@ -283,7 +284,7 @@ int oracle_init_null(oracle_state *s, double a, double r_obs, double inc,
   if (!s || nx <= 0 || ny <= 0 || (uint64_t)nx * (uint64_t)ny != s->n) return 1;
   if (!(fabs(a) <= 1.0) || !(r_obs > 1.0 + sqrt(1.0 - a * a))) return 1;
   double ae = -a;
-  s->a_eff = ae; s->kind = ORACLE_NULL; s->reversed = 1;
+  s->a_eff = ae; s->kind = ORACLE_NULL; s->reversed = 1; s->coords = ORACLE_KS;
   double si = sin(inc), ci = cos(inc);
   double nvec[3] = { si, 0.0, ci }, ea[3] = { 0.0, 1.0, 0.0 }, eb[3] = { -ci, 0.0, si };
 #pragma omp parallel for schedule(static)
@@ -311,7 +312,7 @@ int oracle_init_null(oracle_state *s, double a, double r_obs, double inc,
 int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renorm)
 {
   if (!s || !xu8 || n == 0 || n > s->n || !(fabs(a) <= 1.0)) return 1;
-  s->a_eff = a; s->kind = ORACLE_TIMELIKE; s->reversed = 0;
+  s->a_eff = a; s->kind = ORACLE_TIMELIKE; s->reversed = 0; s->coords = ORACLE_KS;
   for (uint64_t k = 0; k < n; ++k) {
     for (int m = 0; m < 8; ++m) s->q[m][k] = xu8[k * 8 + m];
     if (renorm) s->q[4][k] = solve_ut(a, &xu8[k * 8 + 1], &xu8[k * 8 + 5], 1.0);
@@ -330,13 +331,15 @@ static int all_finite(const double y[8])
   return 1;
 }
 
-static void integrate_one(double a, double y[8], double *lambda, int32_t *status, int32_t *nsteps,
-                          double lambda_end, const oracle_step_control *sc)
+static void integrate_one(double a, int32_t coords, double y[8], double *lambda, int32_t *status,
+                          int32_t *nsteps, double lambda_end, const oracle_step_control *sc)
 {
   double r_plus = 1.0 + sqrt(1.0 - a * a);
   double dir = (double)sc->dir;
   while (*status == ORACLE_ACTIVE) {
-    double r = oracle_ks_r(a, y[1], y[2], y[3]);
+    /* the radius of the stopping tests and of the step rule is the same scalar in both systems: the
+       KS r of eq. (5) "is identical to" the BL r, which is a coordinate there */
+    double r = (coords == ORACLE_BL) ? y[1] : oracle_ks_r(a, y[1], y[2], y[3]);
     if (!isfinite(r) || !all_finite(y)) { *status = ORACLE_INVALID; break; }
     if (r < sc->capture_factor * r_plus) { *status = ORACLE_CAPTURED; break; }
     if (r > sc->r_escape)                { *status = ORACLE_ESCAPED;  break; }
@@ -344,7 +347,8 @@ static void integrate_one(double a, double y[8], double *lambda, int32_t *status
     if (dir * (lambda_end - *lambda) <= 0.0) break; /* stays ACTIVE: resumable */
     double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
     if (fabs(h) > fabs(lambda_end - *lambda)) h = lambda_end - *lambda; /* clip the last step */
-    oracle_rk4_step(a, y, h);
+    if (coords == ORACLE_BL) oracle_bl_rk4_step(a, y, h);
+    else oracle_rk4_step(a, y, h);
     *lambda += h;
     *nsteps += 1;
   }
@@ -363,7 +367,7 @@ int oracle_integrate(oracle_state *s, uint64_t n, double lambda_end,
     for (int m = 0; m < 8; ++m) y[m] = s->q[m][k];
     int32_t st = s->status[k], ns = s->nsteps[k], ns0 = ns;
     double lam = s->lambda[k];
-    integrate_one(s->a_eff, y, &lam, &st, &ns, lambda_end, sc);
+    integrate_one(s->a_eff, s->coords, y, &lam, &st, &ns, lambda_end, sc);
     for (int m = 0; m < 8; ++m) s->q[m][k] = y[m];
     s->status[k] = st; s->nsteps[k] = ns; s->lambda[k] = lam;
     steps += (uint64_t)(ns - ns0);
@@ -429,7 +433,7 @@ void oracle_trajectory_coordtime(double a, const double y0[7], double h, int64_t
 int oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
                                const oracle_step_control *sc, oracle_stats *stats)
 {
-  if (!s || !sc || n == 0 || n > s->n) return 1;
+  if (!s || !sc || n == 0 || n > s->n || s->coords != ORACLE_KS) return 1;
   if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return 1;
   if (sc->dir != 1 && sc->dir != -1) return 1;
   uint64_t steps = 0, nc = 0, ne = 0, nm = 0, ni = 0, na = 0;
@@ -535,7 +539,7 @@ static void diag_sample(diag_acc *D, double a, int32_t kind, const double y[8])
 int oracle_integrate_diagnostics(oracle_state *s, uint64_t n, double lambda_end,
                                  const oracle_step_control *sc, double *out5n, oracle_stats *stats)
 {
-  if (!s || !sc || !out5n || n == 0 || n > s->n) return 1;
+  if (!s || !sc || !out5n || n == 0 || n > s->n || s->coords != ORACLE_KS) return 1;
   if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return 1;
   if (sc->dir != 1 && sc->dir != -1) return 1;
   uint64_t steps = 0, nc = 0, ne = 0, nm = 0, ni = 0, na = 0;
@@ -580,13 +584,16 @@ int oracle_integrate_diagnostics(oracle_state *s, uint64_t n, double lambda_end,
 }
 
 /* ------------------------------------------------------------------------------------------
- * C8.  Independent Boyer-Lindquist integrator (oracle self-check only).
+ * C8.  Boyer-Lindquist coordinates.
  * PAPER.md:47 eq. (1), M = 1, coordinates X = (t, r, theta, phi):
  *   ds^2 = -(1 - 2r/rho^2) dt^2 - (4 r a sin^2/rho^2) dphi dt + (rho^2/Delta) dr^2 + rho^2 dtheta^2
  *          + (r^2 + a^2 + 2 r a^2 sin^2/rho^2) sin^2 dphi^2 ,
  *   rho^2 = r^2 + a^2 cos^2(theta),  Delta = r^2 - 2 r + a^2.
- * Metric derivatives by 4th-order central differences, inverse by Gauss-Jordan, then the same
- * eq. (8) and eq. (7) routines as above.  Nothing Kerr-Schild specific is used.
+ * The paper prints the metric only (5 elements, 10 derivatives, 20 Christoffel symbols);
+ * here the derivatives are eq. (1) differentiated element by element (quotient rule, nothing regrouped),
+ * the inverse comes from Gauss-Jordan elimination, and eq. (8), eq. (7) are the same generic routines
+ * as for Kerr-Schild.  Nothing Kerr-Schild specific is used.  A second derivative routine takes 4th-order
+ * central differences of the metric, so that the analytic one is pinned by something other than itself.
  * ---------------------------------------------------------------------------------------- */
 void oracle_bl_metric(double a, const double X[4], double g[16])
 {
@@ -599,6 +606,47 @@ void oracle_bl_metric(double a, const double X[4], double g[16])
   g[1 * 4 + 1] = rho2 / Delta;
   g[2 * 4 + 2] = rho2;
   g[3 * 4 + 3] = (r * r + a * a + 2.0 * r * a * a * s2 / rho2) * s2;
+}
+
+void oracle_bl_dmetric(double a, const double X[4], double dg[64])
+{
+  double r = X[1], th = X[2];
+  double s = sin(th), c = cos(th), s2 = s * s, s4 = s2 * s2, a2 = a * a;
+  double rho2 = r * r + a2 * c * c, rho4 = rho2 * rho2, Delta = r * r - 2.0 * r + a2;
+  double rho2_r = 2.0 * r, rho2_th = -2.0 * a2 * s * c, Delta_r = 2.0 * r - 2.0;
+  for (int k = 0; k < 64; ++k) dg[k] = 0.0;
+  double *dr = &dg[1 * 16], *dt = &dg[2 * 16];          /* d/dr and d/dtheta; d/dt = d/dphi = 0 */
+  /* g_tt = -1 + 2r/rho2 */
+  dr[0 * 4 + 0] = 2.0 / rho2 - 2.0 * r * rho2_r / rho4;
+  dt[0 * 4 + 0] = -2.0 * r * rho2_th / rho4;
+  /* g_tphi = -2 r a s2 / rho2 */
+  dr[0 * 4 + 3] = dr[3 * 4 + 0] = -2.0 * a * s2 / rho2 + 2.0 * r * a * s2 * rho2_r / rho4;
+  dt[0 * 4 + 3] = dt[3 * 4 + 0] = -4.0 * r * a * s * c / rho2 + 2.0 * r * a * s2 * rho2_th / rho4;
+  /* g_rr = rho2 / Delta */
+  dr[1 * 4 + 1] = rho2_r / Delta - rho2 * Delta_r / (Delta * Delta);
+  dt[1 * 4 + 1] = rho2_th / Delta;
+  /* g_thth = rho2 */
+  dr[2 * 4 + 2] = rho2_r;
+  dt[2 * 4 + 2] = rho2_th;
+  /* g_phiphi = (r^2 + a^2) s2 + 2 r a^2 s4 / rho2 */
+  dr[3 * 4 + 3] = 2.0 * r * s2 + 2.0 * a2 * s4 / rho2 - 2.0 * r * a2 * s4 * rho2_r / rho4;
+  dt[3 * 4 + 3] = 2.0 * (r * r + a2) * s * c + 8.0 * r * a2 * s2 * s * c / rho2 - 2.0 * r * a2 * s4 * rho2_th / rho4;
+}
+
+void oracle_bl_dmetric_fd(double a, const double X[4], double dg[64])
+{
+  for (int k = 0; k < 64; ++k) dg[k] = 0.0;
+  for (int c = 1; c <= 2; ++c) { /* metric depends on r and theta only */
+    double step = 1e-3 * (c == 1 ? fmax(1.0, fabs(X[1])) : 1.0);
+    double Y[4], g1p[16], g1m[16], g2p[16], g2m[16];
+    memcpy(Y, X, sizeof Y);
+    Y[c] = X[c] + step;       oracle_bl_metric(a, Y, g1p);
+    Y[c] = X[c] - step;       oracle_bl_metric(a, Y, g1m);
+    Y[c] = X[c] + 2.0 * step; oracle_bl_metric(a, Y, g2p);
+    Y[c] = X[c] - 2.0 * step; oracle_bl_metric(a, Y, g2m);
+    for (int k = 0; k < 16; ++k)
+      dg[c * 16 + k] = (8.0 * (g1p[k] - g1m[k]) - (g2p[k] - g2m[k])) / (12.0 * step);
+  }
 }
 
 static void invert4(const double m[16], double inv[16])
@@ -625,18 +673,17 @@ void oracle_bl_accel(double a, const double X[4], const double u[4], double acc[
   double g[16], gi[16], dg[64], Gam[64];
   oracle_bl_metric(a, X, g);
   invert4(g, gi);
-  for (int k = 0; k < 64; ++k) dg[k] = 0.0;
-  for (int c = 1; c <= 2; ++c) { /* metric depends on r and theta only */
-    double step = 1e-3 * (c == 1 ? fmax(1.0, fabs(X[1])) : 1.0);
-    double Y[4], g1p[16], g1m[16], g2p[16], g2m[16];
-    memcpy(Y, X, sizeof Y);
-    Y[c] = X[c] + step;       oracle_bl_metric(a, Y, g1p);
-    Y[c] = X[c] - step;       oracle_bl_metric(a, Y, g1m);
-    Y[c] = X[c] + 2.0 * step; oracle_bl_metric(a, Y, g2p);
-    Y[c] = X[c] - 2.0 * step; oracle_bl_metric(a, Y, g2m);
-    for (int k = 0; k < 16; ++k)
-      dg[c * 16 + k] = (8.0 * (g1p[k] - g1m[k]) - (g2p[k] - g2m[k])) / (12.0 * step);
-  }
+  oracle_bl_dmetric(a, X, dg);
+  christoffel_from(gi, dg, Gam);
+  accel_from(Gam, u, acc);
+}
+
+void oracle_bl_accel_fd(double a, const double X[4], const double u[4], double acc[4])
+{
+  double g[16], gi[16], dg[64], Gam[64];
+  oracle_bl_metric(a, X, g);
+  invert4(g, gi);
+  oracle_bl_dmetric_fd(a, X, dg);
   christoffel_from(gi, dg, Gam);
   accel_from(Gam, u, acc);
 }
@@ -646,6 +693,8 @@ static void bl_deriv(double a, const double y[8], double dy[8])
   for (int m = 0; m < 4; ++m) dy[m] = y[4 + m];
   oracle_bl_accel(a, &y[0], &y[4], &dy[4]);
 }
+
+void oracle_bl_rk4_step(double a, double y[8], double h) { rk4_generic(bl_deriv, a, y, h); }
 
 void oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out)
 {
@@ -657,6 +706,121 @@ void oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps
     rk4_generic(bl_deriv, a, y, h);
     if (s % stride == 0) { memcpy(out + 8 * rec, y, sizeof y); ++rec; }
   }
+}
+
+/* E = -u_t, L_z = u_phi, Carter's Q = u_theta^2 + cos^2(theta) [a^2 (mu^2 - E^2) + L_z^2 / sin^2(theta)]
+   (Carter 1968; the paper's Table 1 lists Phi = L_z/E and Q/E^2), u.u = g_ab u^a u^b;
+   indices lowered with eq. (1). */
+void oracle_bl_invariants_one(double a, int32_t kind, const double y[8], double out[4])
+{
+  double g[16], ulow[4];
+  const double *u = &y[4];
+  oracle_bl_metric(a, &y[0], g);
+  for (int i = 0; i < 4; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < 4; ++j) s += g[i * 4 + j] * u[j];
+    ulow[i] = s;
+  }
+  double norm = 0.0;
+  for (int i = 0; i < 4; ++i) norm += ulow[i] * u[i];
+  double E = -ulow[0], Lz = ulow[3];
+  double st = sin(y[2]), ct = cos(y[2]);
+  double mu2 = (kind == ORACLE_TIMELIKE) ? 1.0 : 0.0;
+  double Q = ulow[2] * ulow[2] + ct * ct * (a * a * (mu2 - E * E) + Lz * Lz / (st * st));
+  out[0] = E; out[1] = Lz; out[2] = Q; out[3] = norm;
+}
+
+/* T(r) and Phi(r) with dT/dr = 2r/Delta, dPhi/dr = a/Delta (partial fractions over the roots r_+- of Delta;
+   the double root of the extremal case integrates to a pole instead of a logarithm). */
+static void bl_shift(double a, double r, double *T, double *Phi)
+{
+  double d2 = 1.0 - a * a;
+  if (d2 > 0.0) {
+    double rp = 1.0 + sqrt(d2), rm = 1.0 - sqrt(d2);
+    *T = 2.0 / (rp - rm) * (rp * log(fabs(r - rp)) - rm * log(fabs(r - rm)));
+    *Phi = a / (rp - rm) * log(fabs((r - rp) / (r - rm)));
+  } else {
+    *T = 2.0 * log(fabs(r - 1.0)) - 2.0 / (r - 1.0);
+    *Phi = -a / (r - 1.0);
+  }
+}
+
+/* J[i][j] = d(t_KS, x, y, z)_i / d(t_BL, r, theta, phi_BL)_j at the point (r, theta, phi_KS). */
+static void bl_jacobian(double a, double r, double th, double ph_ks, double J[16])
+{
+  double Delta = r * r - 2.0 * r + a * a;
+  double st = sin(th), ct = cos(th), cp = cos(ph_ks), sp = sin(ph_ks);
+  double x = (r * cp - a * sp) * st, y = (r * sp + a * cp) * st;
+  double dph_dr = a / Delta;                    /* d phi_KS / d r at fixed phi_BL */
+  for (int k = 0; k < 16; ++k) J[k] = 0.0;
+  J[0 * 4 + 0] = 1.0;
+  J[0 * 4 + 1] = 2.0 * r / Delta;
+  J[1 * 4 + 1] = cp * st - y * dph_dr;
+  J[2 * 4 + 1] = sp * st + x * dph_dr;
+  J[3 * 4 + 1] = ct;
+  J[1 * 4 + 2] = (r * cp - a * sp) * ct;
+  J[2 * 4 + 2] = (r * sp + a * cp) * ct;
+  J[3 * 4 + 2] = -r * st;
+  J[1 * 4 + 3] = -y;
+  J[2 * 4 + 3] = x;
+}
+
+void oracle_bl_to_ks_one(double a, const double yb[8], double yk[8])
+{
+  double r = yb[1], th = yb[2], T, Phi, J[16];
+  bl_shift(a, r, &T, &Phi);
+  double ph_ks = yb[3] + Phi;
+  yk[0] = yb[0] + T;
+  yk[1] = (r * cos(ph_ks) - a * sin(ph_ks)) * sin(th);
+  yk[2] = (r * sin(ph_ks) + a * cos(ph_ks)) * sin(th);
+  yk[3] = r * cos(th);
+  bl_jacobian(a, r, th, ph_ks, J);
+  for (int i = 0; i < 4; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < 4; ++j) s += J[i * 4 + j] * yb[4 + j];
+    yk[4 + i] = s;
+  }
+}
+
+/* The inverse map: r from eq. (5), theta = arccos(z/r) in [0, pi], phi_KS = arg(x + i y) - arg(r + i a);
+   the velocity solves J u_BL = u_KS (Gauss-Jordan).  On the axis J is singular and the result is not
+   finite: that is the coordinate singularity of the BL system, reported as data. */
+void oracle_ks_to_bl_one(double a, const double yk[8], double yb[8])
+{
+  double r = oracle_ks_r(a, yk[1], yk[2], yk[3]);
+  double c = yk[3] / r;
+  if (c > 1.0) c = 1.0;
+  if (c < -1.0) c = -1.0;
+  double th = acos(c);
+  double ph_ks = atan2(yk[2], yk[1]) - atan2(a, r);
+  double T, Phi, J[16], Ji[16];
+  bl_shift(a, r, &T, &Phi);
+  yb[0] = yk[0] - T; yb[1] = r; yb[2] = th; yb[3] = ph_ks - Phi;
+  bl_jacobian(a, r, th, ph_ks, J);
+  invert4(J, Ji);
+  for (int i = 0; i < 4; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < 4; ++j) s += Ji[i * 4 + j] * yk[4 + j];
+    yb[4 + i] = s;
+  }
+}
+
+int oracle_convert(const oracle_state *src, oracle_state *dst, uint64_t n, int32_t to_coords)
+{
+  if (!src || !dst || n == 0 || n > src->n || n > dst->n) return 1;
+  if (to_coords != ORACLE_KS && to_coords != ORACLE_BL) return 1;
+  if (src->coords == to_coords) return 1;
+  dst->a_eff = src->a_eff; dst->kind = src->kind; dst->reversed = src->reversed; dst->coords = to_coords;
+#pragma omp parallel for schedule(static)
+  for (int64_t k = 0; k < (int64_t)n; ++k) {
+    double yi[8], yo[8];
+    for (int m = 0; m < 8; ++m) yi[m] = src->q[m][k];
+    if (to_coords == ORACLE_BL) oracle_ks_to_bl_one(src->a_eff, yi, yo);
+    else oracle_bl_to_ks_one(src->a_eff, yi, yo);
+    for (int m = 0; m < 8; ++m) dst->q[m][k] = yo[m];
+    dst->lambda[k] = src->lambda[k]; dst->status[k] = src->status[k]; dst->nsteps[k] = src->nsteps[k];
+  }
+  return 0;
 }
 
 int oracle_num_threads(void)

@@ -27,6 +27,7 @@ extern "C" {
 
 enum { ORACLE_ACTIVE = 0, ORACLE_CAPTURED = 1, ORACLE_ESCAPED = 2, ORACLE_MAXSTEPS = 3, ORACLE_INVALID = 4 };
 enum { ORACLE_NULL = 0, ORACLE_TIMELIKE = 1 };
+enum { ORACLE_KS = 0, ORACLE_BL = 1 };   /* coordinates of a state: Cartesian Kerr-Schild / Boyer-Lindquist */
 
 typedef struct {
   double  *q[8];      /* t,x,y,z,u^t,u^x,u^y,u^z : n doubles each (SoA)             */
@@ -37,6 +38,9 @@ typedef struct {
   double   a_eff;     /* spin used by the integrator (= -a for reversed rays)       */
   int32_t  kind;      /* ORACLE_NULL / ORACLE_TIMELIKE (nominal mu^2 for Carter Q)  */
   int32_t  reversed;  /* 1: time-reversed ray of a backward trace                   */
+  int32_t  coords;    /* ORACLE_KS: q = t,x,y,z,u^t,u^x,u^y,u^z ; ORACLE_BL: q = t,r,theta,phi,u^t,u^r,u^theta,u^phi.
+                         oracle_integrate and oracle_invariants follow it; the coordinate-time and
+                         diagnostics drivers accept ORACLE_KS only                   */
 } oracle_state;
 
 typedef struct {
@@ -89,10 +93,25 @@ int    oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
 int    oracle_integrate_diagnostics(oracle_state *s, uint64_t n, double lambda_end,
                                     const oracle_step_control *sc, double *out5n, oracle_stats *stats);
 
-/* ---- independent Boyer-Lindquist integrator (self-check only; eq. 1) ---- */
+/* ---- Boyer-Lindquist coordinates (eq. 1): the second coordinate system of the paper's
+   benchmark (Table 2 "BL" rows) and an independent check of the KS integrator ---- */
 void   oracle_bl_metric(double a, const double X[4], double g[16]);                 /* X = t,r,theta,phi  */
-void   oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4]);
+void   oracle_bl_dmetric(double a, const double X[4], double dg[64]);               /* analytic, dg[c*16+a*4+b] */
+void   oracle_bl_dmetric_fd(double a, const double X[4], double dg[64]);            /* 4th-order central diffs  */
+void   oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4]);    /* eq. (7)-(8), analytic dg */
+void   oracle_bl_accel_fd(double a, const double X[4], const double u[4], double acc[4]); /* same from dmetric_fd   */
+void   oracle_bl_rk4_step(double a, double y[8], double h);
 void   oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out);
+void   oracle_bl_invariants_one(double a, int32_t kind, const double y[8], double out[4]); /* E,Lz,Q,norm */
+/* the coordinate map between the two systems (the paper's Appendix is missing; DESIGN R18):
+     x + i y = (r + i a) sin(theta) e^{i phi_KS},  z = r cos(theta),
+     t_KS = t_BL + T(r),  phi_KS = phi_BL + Phi(r),  dT/dr = 2r/Delta,  dPhi/dr = a/Delta.
+   y_out and y_in are 8-vectors (position, then contravariant velocity). */
+void   oracle_bl_to_ks_one(double a, const double y_bl[8], double y_ks[8]);
+void   oracle_ks_to_bl_one(double a, const double y_ks[8], double y_bl[8]);
+/* whole states: dst arrays are caller-owned, dst->coords = to_coords on return; lambda, status, nsteps,
+   a_eff, kind, reversed are copied.  Returns 1 on bad arguments (src->coords == to_coords included). */
+int    oracle_convert(const oracle_state *src, oracle_state *dst, uint64_t n, int32_t to_coords);
 
 int    oracle_num_threads(void);
 

@@ -1,0 +1,266 @@
+"""Pins of the oracle's Boyer-Lindquist path (eq. (1); Table 2 "BL" rows): metric
+derivatives, acceleration, the KS <-> BL map, invariants, and the driver loop in BL coordinates.  CPU only.
+
+What fixes the numbers here, other than the oracle itself: finite differences of eq. (1); textbook closed
+forms (radial free fall in Schwarzschild, Kepler frequency of circular Kerr orbits); the paper's Table 1
+(spherical photon orbits: r stays constant, max|cos theta| and Delta phi as printed); the Kerr-Schild
+oracle (already pinned) through the coordinate map; Carter's radial potential for the capture mask."""
+import numpy as np
+import pytest
+
+import closed_forms as cf
+import image_helpers as ih
+import oracle
+from conftest import load_table1
+from paper_1706_07062_b200 import inputs
+
+ROWS = load_table1()
+RNG = np.random.default_rng(1706)
+
+
+def random_bl_points(a, n):
+    rp = cf.r_plus(a)
+    r = rp * 1.05 + RNG.uniform(0.0, 1.0, n) ** 2 * 40.0
+    th = RNG.uniform(0.15, np.pi - 0.15, n)
+    ph = RNG.uniform(-np.pi, np.pi, n)
+    return np.stack([np.zeros(n), r, th, ph], axis=1)
+
+
+# ---- derivatives of eq. (1) and the acceleration -------------------------------------------------
+
+@pytest.mark.parametrize("a", [0.0, 0.5, -0.9375, 1.0])
+def test_bl_dmetric_matches_finite_differences_of_eq1(a):
+    for X in random_bl_points(a, 40):
+        X[1] += 0.5 * cf.r_plus(a)      # the differences of rho^2/Delta lose accuracy next to the horizon
+        an, fd = oracle.bl_dmetric(a, X), oracle.bl_dmetric(a, X, fd=True)
+        # element by element, so that a wrong term in a small element cannot hide behind a large one
+        assert np.all(np.abs(an - fd) <= 1e-7 * np.abs(an) + 1e-12 * np.abs(an).max())
+        assert np.array_equal(an, an.transpose(0, 2, 1))          # symmetric in the metric indices
+        assert not an[0].any() and not an[3].any()                # stationary and axisymmetric
+
+
+@pytest.mark.parametrize("a", [0.0, 0.7, -0.99])
+def test_bl_accel_analytic_matches_finite_difference_connection(a):
+    for X in random_bl_points(a, 40):
+        X[1] += 0.5 * cf.r_plus(a)
+        u = RNG.uniform(-1, 1, 4) * np.array([1.0, 1.0, 1.0 / X[1], 1.0 / X[1]])
+        u[0] = RNG.uniform(1, 2)
+        acc, acc_fd = oracle.bl_accel(a, X, u), oracle.bl_accel_fd(a, X, u)
+        assert np.max(np.abs(acc - acc_fd) / (np.abs(acc) + np.abs(acc).max() * 1e-3 + 1e-12)) < 1e-6
+
+
+def test_schwarzschild_radial_free_fall_from_rest_at_infinity():
+    # textbook: E = 1, u^r = -sqrt(2/r), u^t = 1/(1-2/r)  =>  d2r/dtau2 = -1/r^2 exactly,
+    # d2t/dtau2 = -(2/r^2) u^r u^t / (1-2/r), no angular acceleration
+    for r in (3.0, 6.0, 25.0):
+        ur, ut = -np.sqrt(2.0 / r), 1.0 / (1.0 - 2.0 / r)
+        acc = oracle.bl_accel(0.0, [0.0, r, 1.1, 0.3], [ut, ur, 0.0, 0.0])
+        assert abs(acc[1] + 1.0 / r ** 2) < 1e-14
+        assert abs(acc[0] + 2.0 / r ** 2 * ur * ut / (1.0 - 2.0 / r)) < 1e-13
+        assert abs(acc[2]) < 1e-15 and abs(acc[3]) < 1e-15
+
+
+@pytest.mark.parametrize("a,s", [(0.0, 1), (0.7, 1), (0.7, -1), (0.9375, -1), (1.0, 1)])
+def test_circular_equatorial_orbits_have_no_acceleration(a, s):
+    # Bardeen, Press & Teukolsky 1972: Omega = +-1/(r^1.5 +- a); u = u^t (1, 0, 0, Omega) is a geodesic
+    for r in (cf.r_isco(a, s) * 1.2, 9.0, 30.0):
+        omega, E, Lz, ut = cf.circular_orbit(a, r, s)
+        y = np.array([0.0, r, np.pi / 2, 0.4, ut, 0.0, 0.0, omega * ut])
+        acc = oracle.bl_accel(a, y[:4], y[4:])
+        assert np.max(np.abs(acc)) < 1e-14
+        inv = oracle.bl_invariants_one(a, oracle.TIMELIKE, y)
+        assert np.allclose(inv, [E, Lz, 0.0, -1.0], rtol=0, atol=1e-12)
+
+
+# ---- Table 1 of the paper, integrated in BL ------------------------------------------------------
+
+def bl_spherical_photon_state(a, r):
+    phi, q = cf.teo_phi_q(a, r)
+    ut, uphi, uth = cf.equatorial_first_integrals(a, r, 1.0, phi, q)
+    return np.array([0.0, r, np.pi / 2, 0.0, ut, 0.0, uth, uphi]), phi, q
+
+
+@pytest.mark.parametrize("row", [r for r in ROWS if r["label"] != "C"], ids=lambda r: r["label"])
+def test_bl_integrator_reproduces_table1(row):
+    """PAPER.md:174-184 (a = 1).  Orbit C (Phi = 0) runs through the poles, where the BL system is singular
+    (PAPER.md:49): it is the one row this coordinate system cannot do, and is left to the KS tests."""
+    a = 1.0
+    y0, phi, q = bl_spherical_photon_state(a, row["r"])
+    inv = oracle.bl_invariants_one(a, oracle.NULL, y0)
+    assert abs(inv[0] - 1.0) < 1e-13 and abs(inv[1] - phi) < 1e-12 and abs(inv[2] - q) < 1e-11 and abs(inv[3]) < 1e-13
+    h = 1.0 / 512
+    n = int(6.0 / h)
+    tr = oracle.bl_trajectory(a, y0, h, n)
+    c = np.abs(np.cos(tr[:, 2]))
+    i = next(j for j in range(1, n) if c[j] >= c[j - 1] and c[j] > c[j + 1])
+    y_0, y_1, y_2 = c[i - 1], c[i], c[i + 1]
+    peak = y_1 - (y_2 - y_0) ** 2 / (8.0 * (y_0 - 2.0 * y_1 + y_2))
+    assert abs(peak - row["maxcos"]) < 6e-5
+    assert np.max(np.abs(tr[: i + 1, 1] - row["r"])) < 1e-6                    # spherical: r stays put
+    z = np.cos(tr[:, 2])
+    k = next((j for j in range(1, n) if z[j] < 0.0 <= z[j + 1]), None)
+    if k is not None:
+        w = -z[k] / (z[k + 1] - z[k])
+        dphi = tr[k, 3] + w * (tr[k + 1, 3] - tr[k, 3]) - tr[0, 3]
+        assert abs(dphi - row["dphi"]) < 2e-3 * max(1.0, abs(row["dphi"]))
+
+
+# ---- the coordinate map ---------------------------------------------------------------------------
+
+@pytest.mark.parametrize("a", [0.0, 0.5, -0.9375, 1.0, -1.0])
+def test_shift_functions_have_the_stated_derivatives(a):
+    # dt_KS = dt_BL + (2r/Delta) dr ; dphi_KS = dphi_BL + (a/Delta) dr   (DESIGN R18)
+    for r in (2.5, 4.0, 17.0):
+        d = 1e-4
+        yp = oracle.bl_to_ks_one(a, [0.0, r + d, np.pi / 2, 0.0, 0, 0, 0, 0])
+        ym = oracle.bl_to_ks_one(a, [0.0, r - d, np.pi / 2, 0.0, 0, 0, 0, 0])
+        delta = r * r - 2 * r + a * a
+        assert abs((yp[0] - ym[0]) / (2 * d) - 2 * r / delta) < 1e-6
+        phi = lambda y, rr: np.arctan2(y[2], y[1]) - np.arctan2(a, rr)
+        dphi = (phi(yp, r + d) - phi(ym, r - d)) / (2 * d)
+        assert abs(dphi - a / delta) < 1e-6
+    if a == 0.0:   # Eddington-Finkelstein: t_KS = t + 2 ln|r - 2|
+        assert abs(oracle.bl_to_ks_one(0.0, [1.5, 7.0, 1.0, 0.2, 0, 0, 0, 0])[0] - (1.5 + 2 * np.log(5.0))) < 1e-14
+
+
+@pytest.mark.parametrize("a", [0.0, 0.6, -0.9375, 1.0])
+def test_map_round_trip_and_agreement_with_the_test_suites_own_map(a):
+    for X in random_bl_points(a, 25):
+        u = RNG.uniform(-1, 1, 4)
+        yb = np.concatenate([X, u])
+        yk = oracle.bl_to_ks_one(a, yb)
+        back = oracle.ks_to_bl_one(a, yk)
+        back[3] = yb[3] + np.angle(np.exp(1j * (back[3] - yb[3])))      # phi is an angle
+        assert np.max(np.abs(back - yb) / np.maximum(1.0, np.abs(yb))) < 1e-10
+        if abs(a) < 1.0:
+            ref, _ = cf.bl_to_ks(a, X, u)      # written independently in closed_forms.py
+            assert np.max(np.abs(ref - yk) / np.maximum(1.0, np.abs(ref))) < 1e-13
+
+
+@pytest.mark.parametrize("kind", [oracle.NULL, oracle.TIMELIKE])
+def test_invariants_are_the_same_in_both_systems(kind):
+    # E, L_z, Q, u.u are scalars: the KS evaluation (pinned by Table 1) fixes the BL one and the velocity map
+    a = 0.8
+    for X in random_bl_points(a, 60):
+        u = RNG.uniform(-1, 1, 4) * np.array([1.0, 1.0, 1.0 / X[1], 1.0 / X[1]])
+        yb = np.concatenate([X, u])
+        ib = oracle.bl_invariants_one(a, kind, yb)
+        ik = oracle.invariants_one(a, kind, oracle.bl_to_ks_one(a, yb))
+        # Q carries the nominal mu^2, identical on both sides
+        assert np.max(np.abs(ib - ik) / np.maximum(1.0, np.abs(ik))) < 1e-11
+
+
+def test_convert_whole_state_and_argument_checks():
+    cfg = inputs.CFG3_NULL.scaled(12, 10)
+    ks = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    bl = oracle.convert(ks, oracle.BL)
+    assert (bl.coords, bl.a_eff, bl.kind, bl.reversed) == (oracle.BL, ks.a_eff, ks.kind, ks.reversed)
+    assert np.allclose(bl.q[1], [oracle.ks_r(ks.a_eff, *ks.q[1:4, k]) for k in range(ks.n)], rtol=1e-15)
+    assert (bl.q[5] < 0).all()              # the reversed rays move inward
+    for x, y in zip(oracle.invariants(ks), oracle.invariants(bl)):
+        assert np.max(np.abs(x - y) / np.maximum(1.0, np.abs(x))) < 1e-9
+    ks2 = oracle.convert(bl, oracle.KS)
+    assert np.max(np.abs(ks2.q - ks.q) / np.maximum(1.0, np.abs(ks.q))) < 1e-12
+    with pytest.raises(ValueError):
+        oracle.convert(ks, oracle.KS)
+    sc = oracle.step_control(mode=1, eta=0.01, r_escape=1100.0, max_steps=10)
+    with pytest.raises(Exception):
+        oracle.integrate_coordtime(bl, 10.0, sc)
+
+
+# ---- the driver loop in BL coordinates ------------------------------------------------------------
+
+# Steps must not straddle Delta = 0, where eq. (1) is singular ("coordinate singularities at
+# the event horizons"): with h = eta r and |dr/dlambda| up to ~3 near the horizon, the capture radius needs
+# a margin of ~3 eta.  Every BL run of the suite uses capture_factor = 1.03 (DESIGN R20); the KS run it is
+# compared with uses the same value, so that step counts are comparable.
+BL_CAPTURE = 1.03
+
+
+def run_image(cfg, coords, eta=None, lambda_end=float("inf"), r_escape=None):
+    s0 = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    if coords == oracle.BL:
+        s0 = oracle.convert(s0, oracle.BL)
+    s = s0.copy()
+    sc = oracle.step_control(mode=1, eta=cfg.eta if eta is None else eta, capture_factor=BL_CAPTURE,
+                             r_escape=cfg.r_escape if r_escape is None else r_escape, max_steps=cfg.max_steps * 8)
+    stats = oracle.integrate(s, lambda_end, sc)
+    return s0, s, stats
+
+
+@pytest.mark.parametrize("cfg", [inputs.CFG3_NULL.scaled(40, 32), inputs.CFG2_NULL.scaled(24, 24),
+                                 inputs.CFG1_NULL.scaled(20, 20)], ids=lambda c: c.name)
+def test_bl_image_agrees_with_ks_image_and_with_carters_potential(cfg):
+    k0, k1, kstats = run_image(cfg, oracle.KS)
+    b0, b1, bstats = run_image(cfg, oracle.BL)
+    d, mask = ih.classify_image(cfg, k0)
+    outside = d > 1e-3
+    assert outside.mean() > 0.98
+    assert np.array_equal(b1.status[outside], k1.status[outside])
+    assert np.array_equal((b1.status == oracle.CAPTURED)[outside], mask[outside])
+    assert bstats["n_invalid"] == 0 and bstats["n_active"] == 0 and bstats["n_maxsteps"] == 0
+    # the same geodesics, the same step rule h = eta r: step counts differ by truncation error only
+    assert np.max(np.abs(b1.nsteps - k1.nsteps)[outside]) <= 1
+    # constants of motion are kept to the accuracy of the scheme in either system
+    esc = outside & (b1.status == oracle.ESCAPED)
+    # (rays that pass close to the axis lose accuracy in BL: hence median and maximum)
+    for x0, x1 in zip(oracle.invariants(b0), oracle.invariants(b1)):
+        rel = np.abs(x1 - x0)[esc] / np.maximum(1.0, np.abs(x0[esc]))
+        assert np.median(rel) < 1e-6 and np.max(rel) < 1e-3
+    # final position of escaped rays with equal step counts: (r, theta) agree to truncation error
+    same = esc & (b1.nsteps == k1.nsteps)
+    kb = oracle.convert(k1, oracle.BL)
+    assert same.sum() > 0.9 * esc.sum()
+    er, eth = (np.abs(kb.q[1] - b1.q[1]) / kb.q[1])[same], np.abs(kb.q[2] - b1.q[2])[same]
+    assert np.median(er) < 1e-6 and np.max(er) < 1e-2      # worst: strongly lensed rays near the axis (cfg2, i = 17 deg)
+    assert np.median(eth) < 1e-7 and np.max(eth) < 1e-3
+
+
+def test_bl_driver_is_fourth_order():
+    """All rays stopped at the same affine parameter (past the hole, before the escape radius): halving eta
+    shrinks the distance to a much finer Kerr-Schild run 16-fold, in the coordinates that the map relates
+    point by point, t and phi included (the finite shifts T(r), Phi(r) of the map enter here)."""
+    cfg = inputs.CFG2_NULL.scaled(6, 6)
+    lam = 1900.0
+    _, k1, _ = run_image(cfg, oracle.KS, 0.04 / 16, lambda_end=lam, r_escape=float("inf"))
+    ref = oracle.convert(k1, oracle.BL)
+    errs = []
+    for eta in (0.04, 0.02):
+        _, b1, _ = run_image(cfg, oracle.BL, eta, lambda_end=lam, r_escape=float("inf"))
+        live = (b1.status == oracle.ACTIVE) & (k1.status == oracle.ACTIVE)
+        assert live.sum() >= 20 and np.allclose(b1.lam[live], lam) and np.allclose(k1.lam[live], lam)
+        dq = b1.q[:4, live] - ref.q[:4, live]
+        dq[3] = np.angle(np.exp(1j * dq[3]))
+        dq[1] /= ref.q[1, live]
+        errs.append(np.median(np.abs(dq), axis=1))
+    ratio = errs[0] / errs[1]
+    assert np.all(ratio > 10.0) and np.all(ratio < 24.0), (errs, ratio)
+    assert np.all(errs[1] < 1e-3)
+
+
+def test_bl_stopping_rules_and_resume():
+    cfg = inputs.CFG1_NULL.scaled(10, 10)
+    ks = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    bl = oracle.convert(ks, oracle.BL)
+    sc = oracle.step_control(mode=1, eta=0.01, capture_factor=BL_CAPTURE, r_escape=cfg.r_escape, max_steps=20000)
+    one = bl.copy()
+    oracle.integrate(one, float("inf"), sc)
+    two = bl.copy()
+    oracle.integrate(two, 60.0, sc)
+    assert (two.status == oracle.ACTIVE).all() and np.allclose(two.lam, 60.0, rtol=0, atol=1e-12)
+    oracle.integrate(two, float("inf"), sc)
+    assert np.array_equal(one.status, two.status)
+    # the clipped step at lambda = 60 shifts the later step sequence: same geodesic to truncation error
+    esc = one.status == oracle.ESCAPED
+    assert np.max(np.abs(one.nsteps - two.nsteps)) <= 1
+    for x, y in zip(oracle.invariants(one), oracle.invariants(two)):
+        assert np.median(np.abs(x - y)[esc]) < 1e-6
+    few = bl.copy()
+    st = oracle.integrate(few, float("inf"), oracle.step_control(mode=1, eta=0.01, r_escape=cfg.r_escape, max_steps=7))
+    assert (few.status == oracle.MAXSTEPS).all() and (few.nsteps == 7).all() and st["steps"] == 700
+    # a ray that starts on the axis has no finite BL velocity: INVALID at the first test, never stepped
+    axis = oracle.init_null(0.5, 100.0, 0.0, 1e-30, 1e-30, 1, 1)
+    axis.q[1:3, 0] = 0.0
+    ab = oracle.convert(axis, oracle.BL)
+    st = oracle.integrate(ab, float("inf"), sc)
+    assert ab.status[0] == oracle.INVALID and st["steps"] == 0
