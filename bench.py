@@ -191,7 +191,9 @@ def run_gpu(args):
     cfg = workload_config(args.workload)
     prec = gray2.F64 if args.dtype == "f64" else gray2.F32
     coord = args.form == "coordtime"
-    flops_per_step = gray2.flops_per_step_coordtime(prec) if coord else gray2.flops_per_step(prec)
+    bl = args.form == "bl"          # Boyer-Lindquist variant (Table 2 "BL" rows): init -> convert -> integrate
+    flops_per_step = (gray2.flops_per_step_coordtime(prec) if coord else
+                      gray2.flops_per_step_bl(prec) if bl else gray2.flops_per_step(prec))
     integrate = gray2.integrate_coordtime if coord else gray2.integrate
     props = torch.cuda.get_device_properties(local)
     n_sms = props.multi_processor_count
@@ -203,13 +205,15 @@ def run_gpu(args):
     sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
                             capture_factor=cfg.capture_factor)
     st = gray2.State.empty(cfg.n, prec)
+    st_ks = gray2.State.empty(cfg.n, prec) if bl else st
     stats = gray2.new_stats()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     def one_step(ev=None):
         if ev: ev[0].record(stream)
-        gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st)
+        gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st_ks)
+        if bl: gray2.convert(st_ks, gray2.BL, out=st)
         if ev: ev[1].record(stream)
         integrate(st, INF, sc, stats=stats)
         if ev: ev[2].record(stream)
@@ -260,10 +264,11 @@ def run_gpu(args):
     bounds = [(cfg.n * c // n_chunks, cfg.n * (c + 1) // n_chunks) for c in range(n_chunks)]
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
     host_in_np = host_in.numpy()
-    parts, host_out, chunk_stats = [], [], []
+    parts, parts_ks, host_out, chunk_stats = [], [], [], []
     for lo, hi in bounds:
         m = hi - lo
         parts.append(gray2.State.empty(m, prec))
+        if bl: parts_ks.append(gray2.State.empty(m, prec))
         chunk_stats.append(gray2.new_stats())
         host_out.append(dict(q=torch.empty((8, m), dtype=st.q.dtype).pin_memory(),
                              lam=torch.empty(m, dtype=torch.float64).pin_memory(),
@@ -278,8 +283,14 @@ def run_gpu(args):
         for c, (lo, hi) in enumerate(bounds):
             part, ho = parts[c], host_out[c]
             with torch.cuda.stream(streams[c % 2]):
-                gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=part)   # H2D inside (explicit 8-vectors)
-                part.kind, part.reversed = gray2.NULL, 1
+                if bl:
+                    ks = parts_ks[c]
+                    gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=ks)
+                    ks.kind, ks.reversed = gray2.NULL, 1
+                    gray2.convert(ks, gray2.BL, out=part)
+                else:
+                    gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=part)   # H2D inside (explicit 8-vectors)
+                    part.kind, part.reversed = gray2.NULL, 1
                 integrate(part, INF, sc, stats=chunk_stats[c])
                 inv = gray2.invariants(part)
                 ho["q"].copy_(part.q, non_blocking=True); ho["lam"].copy_(part.lam, non_blocking=True)
@@ -332,11 +343,11 @@ def run_gpu(args):
                        "parallelism": "independent image per GPU, no collective"},
             "clocks": clocks,
             "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "gray2_init_timelike(host 8-vectors) -> gray2_integrate -> gray2_invariants -> D2H of state, invariants, stats",
+                    "api": "gray2_init_timelike(host 8-vectors) -> %sgray2_integrate -> gray2_invariants -> D2H of state, invariants, stats" % ("gray2_convert -> " if bl else ""),
                     "chunks": n_chunks, "streams": 2},
-            "gpu_launches": 4 * args.steps,
+            "gpu_launches": (5 if bl else 4) * args.steps,
             "roofline": {"bound": "alu", "kernel": ("integrate_kernel<double%s>" if prec == gray2.F64 else "integrate_kernel_f32x2<%s>") % (
-                             ", coordinate time" if coord else ("" if prec == gray2.F64 else "affine")),
+                             ", coordinate time" if coord else ", Boyer-Lindquist" if bl else ("" if prec == gray2.F64 else "affine")),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": NCU_DRAM_BYTES.get((args.workload, args.dtype, args.form)),
                          "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_integrate_*_v3.txt)",
@@ -364,8 +375,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--form", default="affine", choices=["affine", "coordtime"],
-                    help="affine: gray2_integrate (eq. 13-14); coordtime: gray2_integrate_coordtime (eq. 18)")
+    ap.add_argument("--form", default="affine", choices=["affine", "coordtime", "bl"],
+                    help="affine: gray2_integrate (eq. 13-14); coordtime: gray2_integrate_coordtime (eq. 18); "
+                         "bl: gray2_integrate on Boyer-Lindquist states (eq. 1; the paper's Table 2 BL rows)")
     ap.add_argument("--workload", default="cfg3", choices=["cfg1", "cfg2", "cfg3", "cfg5"])
     ap.add_argument("--oracle-side", type=int, default=128, help="oracle sample: side x side rays of the same field of view")
     ap.add_argument("--threads", type=int, default=0)

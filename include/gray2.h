@@ -45,6 +45,10 @@ typedef enum { GRAY2_NULL = 0, GRAY2_TIMELIKE = 1 } gray2_kind;        /* nomina
 typedef enum { GRAY2_ACTIVE = 0, GRAY2_CAPTURED = 1, GRAY2_ESCAPED = 2,
                GRAY2_MAXSTEPS = 3, GRAY2_INVALID = 4 } gray2_ray_status;
 typedef enum { GRAY2_OK = 0, GRAY2_EINVAL = 1, GRAY2_ESTATE = 2, GRAY2_ECUDA = 3 } gray2_err;
+/* Coordinates of a state.  GRAY2_KS: Cartesian Kerr-Schild, the system of the method.
+ * GRAY2_BL: Boyer-Lindquist (eq. 1), the second system of the paper's benchmark (Table 2 "BL"
+ * rows): q = t,r,theta,phi,u^t,u^r,u^theta,u^phi. */
+typedef enum { GRAY2_KS = 0, GRAY2_BL = 1 } gray2_coords;
 
 /* State of n geodesics, structure of arrays (8 variables per geodesic; SoA: PAPER.md:316). */
 typedef struct {
@@ -57,6 +61,8 @@ typedef struct {
   int32_t  prec;        /* gray2_precision of q[]                                                       */
   int32_t  kind;        /* gray2_kind (only gray2_invariants reads it: mu^2 inside Carter's Q)          */
   int32_t  reversed;    /* 1: time-reversed ray of a backward trace (physical t = -t, L_z = -L_z)       */
+  int32_t  coords;      /* gray2_coords of q[]; set to GRAY2_KS by gray2_init_*, to the target by         */
+                        /* gray2_convert; gray2_integrate and gray2_invariants follow it                  */
 } gray2_state;
 
 /* Step and stopping rule (DESIGN R4-R6).  For every geodesic with status ACTIVE, repeat:
@@ -99,9 +105,30 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
 /* Integrate the first n geodesics of s (see gray2_step_control).  Only ACTIVE geodesics are touched, so
  * the call is resumable and a second identical call is a no-op.  prec must equal s->prec.
  * device_stats: DEVICE pointer to one gray2_stats, or NULL; it is OVERWRITTEN with the RK4 steps taken
- * by this call and the final status counts over the first n geodesics. */
+ * by this call and the final status counts over the first n geodesics.
+ *
+ * Boyer-Lindquist states (s->coords = GRAY2_BL, made by gray2_convert): the same classic RK4, the same step
+ * and stopping rule with r = q[1] (the BL radius "is identical to" the KS r of eq. 5), the
+ * right-hand side being the Euler-Lagrange equations of eq. (1) (the paper prints the metric only; form
+ * and derivation: csrc/bl_geodesic.cuh).  Eq. (1) is singular on the horizon and on the axis
+ * (PAPER.md:49-51).  Horizon (DESIGN R20): the capture test is applied to the positions of RK4 stages 2-4 and
+ * to the result of the step as well; if one of them has r < capture_factor * r_plus the step is rejected
+ * and the geodesic ends as CAPTURED at the state it had before that step, so no evaluation ever takes place
+ * at Delta <= 0.  Axis (DESIGN R21): nothing is done; with h = eta r a passage closer to the axis than about
+ * 2 eta radians is not resolved and such geodesics come out wrong (the paper's reason for Kerr-Schild
+ * coordinates); a state exactly on the axis has no finite BL velocity and ends as GRAY2_INVALID. */
 int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
                     int32_t prec, gray2_stats *device_stats, void *cuda_stream);
+/* The coordinate map between the two systems for the first n geodesics (the paper's Appendix is missing,
+ * PAPER.md:207; DESIGN R18):  x + i y = (r + i a) sin(theta) e^{i phi_KS},  z = r cos(theta),
+ * t_KS = t_BL + T(r),  phi_KS = phi_BL + Phi(r),  dT/dr = 2r/Delta,  dPhi/dr = a/Delta,  a = src->a_eff,
+ * T and Phi being the partial-fraction logarithms over the roots of Delta (the pole of the double root when
+ * a^2 = 1); velocities are mapped with the Jacobian.  theta in [0, pi], phi in the principal range on output.
+ * Evaluated in double whatever the precision of the state.  dst: caller-owned arrays of the same precision
+ * as src (dst->q.., lambda, status, nsteps, n, prec filled by the caller); on return dst->coords = to_coords
+ * and a_eff, kind, reversed, lambda, status, nsteps are copied.  src and dst must not alias.  On the axis
+ * the BL velocity is not finite (data, not an error).  GRAY2_EINVAL if src is already in to_coords. */
+int gray2_convert(const gray2_state *src, gray2_state *dst, uint64_t n, int32_t to_coords, void *cuda_stream);
 
 /* Coordinate-time form (section 2.2; eq. 18): integrates dv^i/dt = xddot^i - xddot^0 v^i,
  * v^mu = dx^mu/dt with v^0 = 1, six variables, with the same classic RK4 and the same step and stopping
@@ -150,12 +177,16 @@ int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per
  * (FMA = 2 flops, add/mul = 1, each rsqrt/rcp = 1), used for the roofline figure; see DESIGN.md. */
 int gray2_flops_per_step(int32_t prec);
 int gray2_flops_per_step_coordtime(int32_t prec);
+int gray2_flops_per_step_bl(int32_t prec);
 
 /* Diagnostic entry, not one of the four calls of the path: the geodesic right-hand side of eq. (13)-(14)
  * alone, at n points, so that tests can compare it element by element with the oracle's eq. (7).
  * pos (3 n: x.., y.., z..), u (4 n: u^t.., u^x.., u^y.., u^z..), out (4 n): DEVICE arrays, SoA, of
  * double (GRAY2_F64) or float (GRAY2_F32). */
 int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream);
+/* The same for the Boyer-Lindquist right-hand side: pos (2 n: r.., theta..), u (4 n: u^t.., u^r.., u^theta..,
+ * u^phi..), out (4 n). */
+int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream);
 
 /* Diagnostic entry: FMA-only probe kernel (8 independent chains per thread) for measuring the attainable
  * FMA rate of the FP64 / FP32 pipe.  register_operands = 0: multiplier and addend are immediates (best

@@ -81,6 +81,7 @@ def lib():
         _lib.oracle_bl_dmetric.argtypes = [d, p, p]
         _lib.oracle_bl_dmetric_fd.argtypes = [d, p, p]
         _lib.oracle_bl_rk4_step.argtypes = [d, p, d]
+        _lib.oracle_bl_rk4_step_guarded.argtypes = [d, p, d, d]
         _lib.oracle_bl_invariants_one.argtypes = [d, C.c_int32, p, p]
         _lib.oracle_bl_to_ks_one.argtypes = [d, p, p]
         _lib.oracle_ks_to_bl_one.argtypes = [d, p, p]
@@ -346,6 +347,13 @@ def bl_rk4_step(a, y, h):
     y = _vec(y, 8).copy()
     lib().oracle_bl_rk4_step(a, _ptr(y), h)
     return y
+
+
+def bl_rk4_step_guarded(a, y, h, r_capture):
+    """(violated, y_new): y_new == y when a stage position had r < r_capture."""
+    y = _vec(y, 8).copy()
+    rc = lib().oracle_bl_rk4_step_guarded(a, _ptr(y), h, r_capture)
+    return bool(rc), y
 
 
 def bl_invariants_one(a, kind, y):

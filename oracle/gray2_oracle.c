@@ -347,8 +347,10 @@ static void integrate_one(double a, int32_t coords, double y[8], double *lambda,
     if (dir * (lambda_end - *lambda) <= 0.0) break; /* stays ACTIVE: resumable */
     double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
     if (fabs(h) > fabs(lambda_end - *lambda)) h = lambda_end - *lambda; /* clip the last step */
-    if (coords == ORACLE_BL) oracle_bl_rk4_step(a, y, h);
-    else oracle_rk4_step(a, y, h);
+    if (coords == ORACLE_BL) {
+      /* a stage at r < capture radius: CAPTURED at the state before this step (DESIGN R20) */
+      if (oracle_bl_rk4_step_guarded(a, y, h, sc->capture_factor * r_plus)) { *status = ORACLE_CAPTURED; break; }
+    } else oracle_rk4_step(a, y, h);
     *lambda += h;
     *nsteps += 1;
   }
@@ -695,6 +697,31 @@ static void bl_deriv(double a, const double y[8], double dy[8])
 }
 
 void oracle_bl_rk4_step(double a, double y[8], double h) { rk4_generic(bl_deriv, a, y, h); }
+
+/* The same classic RK4 step with the capture test applied to the positions at which stages 2-4 are
+ * evaluated (DESIGN R20): eq. (1) is singular at Delta = 0, so a stage evaluated at or beyond
+ * the horizon is meaningless, and with h = eta r a geodesic that falls in reaches it within one step of
+ * r = capture_factor r_+.  Returns 1 and leaves y untouched if the radius of a stage position, or of the
+ * result of the step, is below r_capture: the last stored state of a captured ray is then one that only
+ * well-defined evaluations have produced. */
+int oracle_bl_rk4_step_guarded(double a, double y[8], double h, double r_capture)
+{
+  double k1[8], k2[8], k3[8], k4[8], w[8];
+  bl_deriv(a, y, k1);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + 0.5 * h * k1[i];
+  if (w[1] < r_capture) return 1;
+  bl_deriv(a, w, k2);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + 0.5 * h * k2[i];
+  if (w[1] < r_capture) return 1;
+  bl_deriv(a, w, k3);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + h * k3[i];
+  if (w[1] < r_capture) return 1;
+  bl_deriv(a, w, k4);
+  for (int i = 0; i < 8; ++i) w[i] = y[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+  if (w[1] < r_capture) return 1;       /* the result of the step is held to the same test */
+  memcpy(y, w, sizeof w);
+  return 0;
+}
 
 void oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out)
 {

@@ -101,6 +101,9 @@ void   oracle_bl_dmetric_fd(double a, const double X[4], double dg[64]);        
 void   oracle_bl_accel(double a, const double X[4], const double u[4], double acc[4]);    /* eq. (7)-(8), analytic dg */
 void   oracle_bl_accel_fd(double a, const double X[4], const double u[4], double acc[4]); /* same from dmetric_fd   */
 void   oracle_bl_rk4_step(double a, double y[8], double h);
+/* the step of oracle_integrate on BL states: returns 1 and leaves y untouched when the position of a
+   stage, or the result of the step, has r < r_capture (the ray then ends as CAPTURED, DESIGN R20) */
+int    oracle_bl_rk4_step_guarded(double a, double y[8], double h, double r_capture);
 void   oracle_bl_trajectory(double a, const double y0[8], double h, int64_t nsteps, int64_t stride, double *out);
 void   oracle_bl_invariants_one(double a, int32_t kind, const double y[8], double out[4]); /* E,Lz,Q,norm */
 /* the coordinate map between the two systems (the paper's Appendix is missing; DESIGN R18):

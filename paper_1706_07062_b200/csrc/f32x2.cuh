@@ -43,9 +43,22 @@ template <> struct fastmath<f32x2> {
   }
 };
 
+// componentwise minimum (declared in bl_geodesic.cuh for the scalar types)
+template <typename T> __device__ __forceinline__ T min_(T a, T b);
+template <> __device__ __forceinline__ f32x2 min_<f32x2>(f32x2 a, f32x2 b) {
+  return f32x2(fminf(a.v.x, b.v.x), fminf(a.v.y, b.v.y));
+}
+
 template <int C> __device__ __forceinline__ float half_of(f32x2 a) { return C == 0 ? a.v.x : a.v.y; }
 template <int C> __device__ __forceinline__ void set_half(f32x2 &a, float s) {
   if (C == 0) a.v.x = s; else a.v.y = s;
+}
+
+// copy half C of every variable of a packed ray
+template <int C> __device__ __forceinline__ void copy_half(Ray<f32x2> &d, const Ray<f32x2> &s) {
+  set_half<C>(d.t, half_of<C>(s.t)); set_half<C>(d.x, half_of<C>(s.x)); set_half<C>(d.y, half_of<C>(s.y));
+  set_half<C>(d.z, half_of<C>(s.z)); set_half<C>(d.u0, half_of<C>(s.u0)); set_half<C>(d.u1, half_of<C>(s.u1));
+  set_half<C>(d.u2, half_of<C>(s.u2)); set_half<C>(d.u3, half_of<C>(s.u3));
 }
 
 }  // namespace gray2

@@ -73,6 +73,7 @@ int check_state(const gray2_state *s, const char *who) {
     if (!s->q[m]) return fail(GRAY2_EINVAL, "%s: state q[%d] is NULL", who, m);
   if (!s->lambda || !s->status || !s->nsteps) return fail(GRAY2_EINVAL, "%s: lambda/status/nsteps is NULL", who);
   if (s->prec != GRAY2_F64 && s->prec != GRAY2_F32) return fail(GRAY2_EINVAL, "%s: unknown precision %d", who, s->prec);
+  if (s->coords != GRAY2_KS && s->coords != GRAY2_BL) return fail(GRAY2_EINVAL, "%s: unknown coordinates %d", who, s->coords);
   return GRAY2_OK;
 }
 
@@ -119,7 +120,7 @@ cudaError_t launch_integrate_x2(const gray2_state *s, uint64_t n, const gray2::S
 struct LaunchChoice { int threads, blocks; };
 
 // Compiled variants of the affine-parameter integrator; the first entry of each list is the default
-// and the only one compiled for the coordinate-time form.  FP32: the first three entries run two
+// and the only one compiled for the coordinate-time form and for the Boyer-Lindquist form.  FP32: the first three entries run two
 // geodesics per thread (integrate_kernel_f32x2), the last two one per thread (integrate_kernel<float>);
 // every variant gives bit-identical results.
 constexpr int kNumVariants = 5;
@@ -133,12 +134,14 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
   *found = true;
   if constexpr (sizeof(T) == 8) {
     if (form == 1) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, st);
+    if (form == 2) return launch_integrate<T, 128, 3, 2>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
     GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(128, 2)
 #undef GRAY2_VARIANT
   } else {
     if (form == 1) return launch_integrate_x2<256, 2, 1>(s, n, p, q, steps, st);
+    if (form == 2) return launch_integrate_x2<256, 2, 2>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT_X2(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT(TH, BL) \
@@ -240,6 +243,7 @@ const char *gray2_version(void) { return "gray2-b200 0.1 (sm_100a)"; }
 
 int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double Wa, double Wb,
                     int32_t nx, int32_t ny, void *cuda_stream) {
+  if (s) s->coords = GRAY2_KS;
   int rc = check_state(s, "gray2_init_null");
   if (rc) return rc;
   if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_null: |a| must be <= 1 (got %g)", a);
@@ -248,7 +252,7 @@ int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double W
   if (!(r_obs > 1.0 + sqrt(1.0 - a * a))) return fail(GRAY2_EINVAL, "gray2_init_null: r_obs must exceed r_plus");
   if (!(Wa > 0.0) || !(Wb > 0.0) || !isfinite(inc)) return fail(GRAY2_EINVAL, "gray2_init_null: bad field of view or inclination");
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  s->a_eff = -a; s->kind = GRAY2_NULL; s->reversed = 1;
+  s->a_eff = -a; s->kind = GRAY2_NULL; s->reversed = 1; s->coords = GRAY2_KS;
   unsigned grid = (unsigned)((s->n + 255) / 256);
   if (s->prec == GRAY2_F64)
     gray2::init_null_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), -a, r_obs, sin(inc), cos(inc), Wa, Wb, nx, ny);
@@ -260,6 +264,7 @@ int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double W
 
 int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t renorm,
                         void *cuda_stream) {
+  if (s) s->coords = GRAY2_KS;
   int rc = check_state(s, "gray2_init_timelike");
   if (rc) return rc;
   if (!host_xu8 || n == 0) return fail(GRAY2_EINVAL, "gray2_init_timelike: host_xu8 is NULL or n == 0");
@@ -290,7 +295,7 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the staging buffer and host_xu8 may be reused on return
   if (e != cudaSuccess) return fail(GRAY2_ECUDA, "gray2_init_timelike: %s", cudaGetErrorString(e));
-  s->a_eff = a; s->kind = GRAY2_TIMELIKE; s->reversed = 0;
+  s->a_eff = a; s->kind = GRAY2_TIMELIKE; s->reversed = 0; s->coords = GRAY2_KS;
   return GRAY2_OK;
 }
 
@@ -308,6 +313,10 @@ static int integrate_common(int form, const char *who, gray2_state *s, uint64_t 
   if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(end) || sc->max_steps < 0)
     return fail(GRAY2_EINVAL, "%s: bad capture_factor / r_escape / end value / max_steps", who);
   if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a_eff| must be <= 1", who);
+  if (s->coords == GRAY2_BL) {
+    if (form != 0) return fail(GRAY2_EINVAL, "%s: needs a Kerr-Schild state (s->coords = GRAY2_KS)", who);
+    form = 2;
+  }
   rc = ensure_scratch();
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -332,6 +341,7 @@ int gray2_integrate_diagnostics(gray2_state *s, uint64_t n, double lambda_end, c
   int rc = check_state(s, who);
   if (rc) return rc;
   if (!sc || !diag) return fail(GRAY2_EINVAL, "%s: step control or diagnostics is NULL", who);
+  if (s->coords != GRAY2_KS) return fail(GRAY2_EINVAL, "%s: needs a Kerr-Schild state (s->coords = GRAY2_KS)", who);
   if (!diag->max_abs_u2 || !diag->cos_peak || !diag->dphi_cycle || !diag->t_zmax1 || !diag->t_zmax2)
     return fail(GRAY2_EINVAL, "%s: a diagnostics array is NULL", who);
   if (n == 0) return fail(GRAY2_EINVAL, "%s: n == 0", who);
@@ -359,10 +369,40 @@ int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, do
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   double mu2 = s->kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
   unsigned grid = (unsigned)((n + 255) / 256);
-  if (s->prec == GRAY2_F64)
+  if (s->coords == GRAY2_BL) {
+    if (s->prec == GRAY2_F64)
+      gray2::invariants_bl_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), n, s->a_eff, mu2, E, Lz, Q, norm);
+    else
+      gray2::invariants_bl_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), n, s->a_eff, mu2, E, Lz, Q, norm);
+  } else if (s->prec == GRAY2_F64)
     gray2::invariants_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), n, s->a_eff, mu2, E, Lz, Q, norm);
   else
     gray2::invariants_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), n, s->a_eff, mu2, E, Lz, Q, norm);
+  CUDA_TRY(cudaGetLastError());
+  return GRAY2_OK;
+}
+
+int gray2_convert(const gray2_state *src, gray2_state *dst, uint64_t n, int32_t to_coords, void *cuda_stream) {
+  int rc = check_state(src, "gray2_convert");
+  if (rc) return rc;
+  if (dst) dst->coords = to_coords;
+  rc = check_state(dst, "gray2_convert");
+  if (rc) return rc;
+  if (src->coords == to_coords) return fail(GRAY2_EINVAL, "gray2_convert: the state is already in those coordinates");
+  if (src->prec != dst->prec) return fail(GRAY2_EINVAL, "gray2_convert: src and dst differ in precision");
+  if (n == 0) return fail(GRAY2_EINVAL, "gray2_convert: n == 0");
+  if (n > src->n || n > dst->n) return fail(GRAY2_ESTATE, "gray2_convert: n exceeds the size of src or dst");
+  if (!(fabs(src->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_convert: |a_eff| must be <= 1");
+  dst->a_eff = src->a_eff; dst->kind = src->kind; dst->reversed = src->reversed;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned grid = (unsigned)((n + 255) / 256);
+  if (to_coords == GRAY2_BL) {
+    if (src->prec == GRAY2_F64) gray2::ks_to_bl_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(src), view_of<double>(dst), n, src->a_eff);
+    else gray2::ks_to_bl_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(src), view_of<float>(dst), n, src->a_eff);
+  } else {
+    if (src->prec == GRAY2_F64) gray2::bl_to_ks_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(src), view_of<double>(dst), n, src->a_eff);
+    else gray2::bl_to_ks_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(src), view_of<float>(dst), n, src->a_eff);
+  }
   CUDA_TRY(cudaGetLastError());
   return GRAY2_OK;
 }
@@ -385,6 +425,22 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
   return GRAY2_OK;
 }
 
+int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream) {
+  if (!pos || !u || !out || n == 0) return fail(GRAY2_EINVAL, "gray2_rhs_bl: NULL pointer or n == 0");
+  if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_rhs_bl: unknown precision");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  unsigned grid = (unsigned)((n + 127) / 128);
+  if (prec == GRAY2_F64) {
+    gray2::SpinConst<double> k{a, a * a, 2.0 * a, 2.0 * a * a};
+    gray2::rhs_bl_kernel<double><<<grid, 128, 0, st>>>(k, n, (const double *)pos, (const double *)u, (double *)out);
+  } else {
+    gray2::SpinConst<float> k{(float)a, (float)(a * a), (float)(2.0 * a), (float)(2.0 * a * a)};
+    gray2::rhs_bl_kernel<float><<<grid, 128, 0, st>>>(k, n, (const float *)pos, (const float *)u, (float *)out);
+  }
+  CUDA_TRY(cudaGetLastError());
+  return GRAY2_OK;
+}
+
 /* Source-level count of ks_geodesic.cuh (FMA = 2, add/mul = 1, rsqrt/rcp = 1; negations and compares free):
  *   radius 16, rest of geometry 23, velocity part 75  ->  114 per right-hand side
  *   4 x 114 + RK4 combination 100 + step rule and lambda update 2 = 558 per step (both precisions). */
@@ -392,6 +448,13 @@ int gray2_flops_per_step(int32_t prec) { (void)prec; return 558; }
 
 /* Coordinate-time form: 4 x (114 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
 int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 562; }
+
+/* Boyer-Lindquist form, source-level count of bl_geodesic.cuh (same conventions):
+ *   sin^2, cos^2, sin cos of theta: reduction 8, series 21 + 22, products 3 -> 54 (double: 10 / 11 terms),
+ *                                   36 (float: 6 / 6 terms)
+ *   rest of the right-hand side 87 (4 of them reciprocals)  ->  141 / 123 per right-hand side
+ *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 666 / 594 per step. */
+int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 594 : 666; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.

@@ -13,6 +13,7 @@
 #include "../../include/gray2.h"
 #include "ks_geodesic.cuh"
 #include "f32x2.cuh"
+#include "bl_geodesic.cuh"
 
 namespace gray2 {
 
@@ -93,7 +94,9 @@ __global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ 
 // the tests are ordered only in the (rare) slow path that classifies and stores a finished ray.
 //
 // FORM: 0 affine parameter (eq. 13-14, eight variables); 1 coordinate time (eq. 18, six variables): the
-// clock `lam` is then t itself, v^i = u^i/u^t on load, and (t, x, 1, v) is stored; `lambda` is untouched.
+// clock `lam` is then t itself, v^i = u^i/u^t on load, and (t, x, 1, v) is stored; `lambda` is untouched;
+// 2 affine parameter in Boyer-Lindquist coordinates (bl_geodesic.cuh): the state is (t, r, theta, phi) and
+// its derivatives, the radius of the step rule and of the stopping tests is the coordinate r itself.
 template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long *queue,
@@ -105,10 +108,12 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
   Ray<T> ray;
   ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = T(0);
   ray.z = T(3);                // idle lanes integrate a harmless dummy state (never stored)
+  if constexpr (FORM == 2) { ray.x = T(3); ray.y = T(1); }
   double lam = 0.0;
   int32_t nst = 0, nst0 = 0;
   uint64_t idx = 0;
   bool have = false;           // this lane holds an ACTIVE geodesic
+  bool cap = false;            // FORM 2: the last step was rejected, a stage reached the capture radius
   bool drained = false;        // warp-uniform: the queue has no more work
   unsigned long long my_steps = 0;
 
@@ -146,24 +151,32 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
     // ---- step all lanes until one of them has to stop ---------------------------------------------
     for (;;) {
       Geometry<T> g;
-      ks_geometry(k, ray.x, ray.y, ray.z, g);
-      T U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+      T U;
+      if constexpr (FORM == 2) {
+        g.r = ray.x;
+        U = bl_probe(ray);
+      } else {
+        ks_geometry(k, ray.x, ray.y, ray.z, g);
+        U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+      }
       // NaN fails every compare; r_escape_fin = min(r_escape, largest finite) so that r = inf fails too
       bool go = (g.r >= p.r_capture) && (g.r <= p.r_escape_fin) && fastmath<T>::finite(U) &&
                 fastmath<T>::finite(ray.t) && (nst < p.max_steps);
       if (CLIP) go = go && (p.dir * (p.lambda_end - lam) > 0.0);
+      if constexpr (FORM == 2) go = go && !cap;
       if (__any_sync(0xffffffffu, have && !go)) {
         if (have && !go) {
           // classify in the order of gray2_step_control and store the state where the test fired
           int32_t st = GRAY2_ACTIVE;    // lambda_end reached: stays ACTIVE (resumable)
           if (!(fastmath<T>::finite(g.r) && fastmath<T>::finite(U) && fastmath<T>::finite(ray.t))) st = GRAY2_INVALID;
-          else if (g.r < p.r_capture) st = GRAY2_CAPTURED;
+          else if (g.r < p.r_capture || cap) st = GRAY2_CAPTURED;
           else if (g.r > p.r_escape) st = GRAY2_ESCAPED;
           else if (nst >= p.max_steps) st = GRAY2_MAXSTEPS;
+          cap = false;
           if constexpr (FORM == 1) ray.t = (T)lam;
           s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
           s.q[4][idx] = ray.u0; s.q[5][idx] = ray.u1; s.q[6][idx] = ray.u2; s.q[7][idx] = ray.u3;
-          if constexpr (FORM == 0) s.lambda[idx] = lam;
+          if constexpr (FORM != 1) s.lambda[idx] = lam;
           s.status[idx] = st; s.nsteps[idx] = nst;
           my_steps += (unsigned long long)(nst - nst0);
           have = false;
@@ -176,10 +189,19 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
         double rem = p.lambda_end - lam;
         if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
       }
-      if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
-      else rk4_step(k, ray, g, h);
-      lam += hd;
-      nst += 1;
+      if constexpr (FORM == 2) {
+        // the step is accepted only if no stage position, and not its result, is inside the capture radius;
+        // otherwise the geodesic ends as CAPTURED at the state it has now (DESIGN R20)
+        Ray<T> nxt;
+        T rmin = rk4_step_bl<T, TrigConst<T>>(k, ray, h, nxt);
+        if (rmin < p.r_capture) cap = true;
+        else { ray = nxt; lam += hd; nst += 1; }
+      } else {
+        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
+        else rk4_step(k, ray, g, h);
+        lam += hd;
+        nst += 1;
+      }
     }
   }
 
@@ -196,6 +218,7 @@ struct PairSlot {
   double lam;
   int32_t nst, nst0;
   bool have;
+  bool cap;     // FORM 2: the last step was rejected, a stage reached the capture radius
 };
 
 template <int C, int FORM>
@@ -216,6 +239,7 @@ __device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n,
     set_half<C>(ray.u2, u2); set_half<C>(ray.u3, u3);
     sl.nst = sl.nst0 = s.nsteps[mine];
     sl.have = true;
+    sl.cap = false;
   }
 }
 
@@ -226,7 +250,7 @@ __device__ __forceinline__ bool slot_may_step(const StepParams<float> &p, const 
   bool go = (r >= p.r_capture) && (r <= p.r_escape_fin) && fastmath<float>::finite(half_of<C>(U)) &&
             fastmath<float>::finite(half_of<C>(ray.t)) && (sl.nst < p.max_steps);
   if (CLIP) go = go && (p.dir * (p.lambda_end - sl.lam) > 0.0);
-  return go;
+  return go && !sl.cap;
 }
 
 template <int C, int FORM>
@@ -236,7 +260,7 @@ __device__ __forceinline__ void store_slot(const StateView<float> &s, const Step
   float r = half_of<C>(g.r), t = half_of<C>(ray.t);
   int32_t st = GRAY2_ACTIVE;
   if (!(fastmath<float>::finite(r) && fastmath<float>::finite(half_of<C>(U)) && fastmath<float>::finite(t))) st = GRAY2_INVALID;
-  else if (r < p.r_capture) st = GRAY2_CAPTURED;
+  else if (r < p.r_capture || sl.cap) st = GRAY2_CAPTURED;
   else if (r > p.r_escape) st = GRAY2_ESCAPED;
   else if (sl.nst >= p.max_steps) st = GRAY2_MAXSTEPS;
   const uint64_t i = sl.idx;
@@ -244,7 +268,7 @@ __device__ __forceinline__ void store_slot(const StateView<float> &s, const Step
   s.q[1][i] = half_of<C>(ray.x); s.q[2][i] = half_of<C>(ray.y); s.q[3][i] = half_of<C>(ray.z);
   s.q[4][i] = half_of<C>(ray.u0); s.q[5][i] = half_of<C>(ray.u1); s.q[6][i] = half_of<C>(ray.u2);
   s.q[7][i] = half_of<C>(ray.u3);
-  if (FORM == 0) s.lambda[i] = sl.lam;
+  if (FORM != 1) s.lambda[i] = sl.lam;
   s.status[i] = st; s.nsteps[i] = sl.nst;
   my_steps += (unsigned long long)(sl.nst - sl.nst0);
   sl.have = false;
@@ -261,7 +285,8 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
   Ray<f32x2> ray;
   ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = f32x2(0.0f);
   ray.z = f32x2(3.0f);         // idle slots integrate a harmless dummy state (never stored)
-  PairSlot A{0, 0.0, 0, 0, false}, B{0, 0.0, 0, 0, false};
+  if constexpr (FORM == 2) { ray.x = f32x2(3.0f); ray.y = f32x2(1.0f); }
+  PairSlot A{0, 0.0, 0, 0, false, false}, B{0, 0.0, 0, 0, false, false};
   bool drained = false;
   unsigned long long my_steps = 0;
 
@@ -281,8 +306,14 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
 
     for (;;) {
       Geometry<f32x2> g;
-      ks_geometry(k, ray.x, ray.y, ray.z, g);
-      f32x2 U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+      f32x2 U;
+      if constexpr (FORM == 2) {
+        g.r = ray.x;
+        U = bl_probe(ray);
+      } else {
+        ks_geometry(k, ray.x, ray.y, ray.z, g);
+        U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+      }
       bool stopA = A.have && !slot_may_step<0, CLIP>(p, g, U, ray, A);
       bool stopB = B.have && !slot_may_step<1, CLIP>(p, g, U, ray, B);
       if (__any_sync(0xffffffffu, stopA || stopB)) {
@@ -297,10 +328,19 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
         if (fabs(hdA) > fabs(remA)) { hdA = remA; h.v.x = (float)remA; }
         if (fabs(hdB) > fabs(remB)) { hdB = remB; h.v.y = (float)remB; }
       }
-      if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
-      else rk4_step(k, ray, g, h);
-      A.lam += hdA; B.lam += hdB;
-      A.nst += 1; B.nst += 1;
+      if constexpr (FORM == 2) {
+        Ray<f32x2> nxt;
+        f32x2 rmin = rk4_step_bl<f32x2, TrigConst<float>>(k, ray, h, nxt);
+        if (rmin.v.x < p.r_capture) A.cap = true;
+        else { copy_half<0>(ray, nxt); A.lam += hdA; A.nst += 1; }
+        if (rmin.v.y < p.r_capture) B.cap = true;
+        else { copy_half<1>(ray, nxt); B.lam += hdB; B.nst += 1; }
+      } else {
+        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
+        else rk4_step(k, ray, g, h);
+        A.lam += hdA; B.lam += hdB;
+        A.nst += 1; B.nst += 1;
+      }
     }
   }
 
@@ -422,6 +462,107 @@ __global__ void invariants_kernel(StateView<T> s, uint64_t n, double a, double m
   double q = P * c * c * (cx * cx + cy * cy) - 2.0 * r * c * (x * cx + y * cy) * cz + r2 * s2 * cz * cz +
              a * a * c * c * (mu2 - e * e);
   E[idx] = e; Lz[idx] = lz; Q[idx] = q; norm[idx] = nn;
+}
+
+// Boyer-Lindquist state: E = -u_t, L_z = u_phi, u_theta = Sigma theta', with eq. (1) in the form
+// ds^2 = -dt^2 + Sigma (dr^2/Delta + dtheta^2) + P sin^2 dphi^2 + A (dt - a sin^2 dphi)^2.
+template <typename T>
+__global__ void invariants_bl_kernel(StateView<T> s, uint64_t n, double a, double mu2, double *__restrict__ E,
+                                     double *__restrict__ Lz, double *__restrict__ Q, double *__restrict__ norm) {
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n) return;
+  double r = (double)s.q[1][idx], th = (double)s.q[2][idx];
+  double u0 = (double)s.q[4][idx], u1 = (double)s.q[5][idx], u2 = (double)s.q[6][idx], u3 = (double)s.q[7][idx];
+  double sn, cs;
+  sincos(th, &sn, &cs);
+  double s2 = sn * sn, c2 = cs * cs, a2 = a * a;
+  double Sig = r * r + a2 * c2, P = r * r + a2, Dl = P - 2.0 * r, A = 2.0 * r / Sig;
+  double om = u0 - a * s2 * u3, W = A * om;
+  double e = u0 - W;
+  double lz = s2 * (P * u3 - a * W);
+  double pth = Sig * u2;
+  E[idx] = e; Lz[idx] = lz;
+  Q[idx] = pth * pth + c2 * (a2 * (mu2 - e * e) + lz * lz / s2);
+  norm[idx] = -u0 * u0 + Sig * (u1 * u1 / Dl + u2 * u2) + P * s2 * u3 * u3 + W * om;
+}
+
+// ---- the coordinate map Kerr-Schild <-> Boyer-Lindquist (DESIGN R18; the paper's Appendix is missing,
+// PAPER.md:207).  x + i y = (r + i a) sin(theta) e^{i phi_KS}, z = r cos(theta), t_KS = t_BL + T(r),
+// phi_KS = phi_BL + Phi(r), dT/dr = 2r/Delta, dPhi/dr = a/Delta.  Always evaluated in double.
+__device__ __forceinline__ void bl_shift(double a, double r, double &T, double &Phi) {
+  double d2 = 1.0 - a * a;
+  if (d2 > 0.0) {
+    double sq = sqrt(d2), rp = 1.0 + sq, rm = 1.0 - sq, w = 0.5 / sq;       // 1/(r_+ - r_-)
+    double lp = log(fabs(r - rp)), lm = log(fabs(r - rm));
+    T = 2.0 * w * (rp * lp - rm * lm);
+    Phi = a * w * (lp - lm);
+  } else {                                                                   // double root r_+ = r_- = 1
+    T = 2.0 * log(fabs(r - 1.0)) - 2.0 / (r - 1.0);
+    Phi = -a / (r - 1.0);
+  }
+}
+
+template <typename T>
+__global__ void ks_to_bl_kernel(StateView<T> src, StateView<T> dst, uint64_t n, double a) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double t = (double)src.q[0][i], x = (double)src.q[1][i], y = (double)src.q[2][i], z = (double)src.q[3][i];
+  double u0 = (double)src.q[4][i], u1 = (double)src.q[5][i], u2 = (double)src.q[6][i], u3 = (double)src.q[7][i];
+  double a2 = a * a, rho2 = x * x + y * y;
+  double w = rho2 + z * z - a2, D = sqrt(w * w + 4.0 * a2 * z * z);
+  double r2 = 0.5 * (w + D), r = sqrt(r2), P = r2 + a2, Dl = P - 2.0 * r;
+  double cs = z / r, sn = sqrt(rho2 / P);
+  // implicit differentiation of eq. (5): r' = [r^2 (x.u) + a^2 z u^z] / (r D)
+  double rd = (r2 * (x * u1 + y * u2 + z * u3) + a2 * z * u3) / (r * D);
+  double thd = (cs * rd - u3) / (r * sn);
+  double phd = (x * u2 - y * u1) / rho2 + a * rd / P;       // d/dlambda of arg(x + i y) - arg(r + i a)
+  double Tr, Phr;
+  bl_shift(a, r, Tr, Phr);
+  dst.q[0][i] = (T)(t - Tr);
+  dst.q[1][i] = (T)r;
+  dst.q[2][i] = (T)atan2(sn, cs);
+  dst.q[3][i] = (T)(atan2(y, x) - atan2(a, r) - Phr);
+  dst.q[4][i] = (T)(u0 - 2.0 * r / Dl * rd);
+  dst.q[5][i] = (T)rd;
+  dst.q[6][i] = (T)thd;
+  dst.q[7][i] = (T)(phd - a / Dl * rd);
+  dst.lambda[i] = src.lambda[i]; dst.status[i] = src.status[i]; dst.nsteps[i] = src.nsteps[i];
+}
+
+template <typename T>
+__global__ void bl_to_ks_kernel(StateView<T> src, StateView<T> dst, uint64_t n, double a) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double t = (double)src.q[0][i], r = (double)src.q[1][i], th = (double)src.q[2][i], ph = (double)src.q[3][i];
+  double u0 = (double)src.q[4][i], rd = (double)src.q[5][i], thd = (double)src.q[6][i], phd = (double)src.q[7][i];
+  double Dl = r * r - 2.0 * r + a * a, Tr, Phr;
+  bl_shift(a, r, Tr, Phr);
+  double sn, cs, sp, cp;
+  sincos(th, &sn, &cs);
+  sincos(ph + Phr, &sp, &cp);
+  double ex = r * cp - a * sp, ey = r * sp + a * cp;         // (x, y) = (ex, ey) sin(theta)
+  double x = ex * sn, y = ey * sn;
+  double phk = phd + a / Dl * rd;                            // d phi_KS / dlambda
+  dst.q[0][i] = (T)(t + Tr);
+  dst.q[1][i] = (T)x;
+  dst.q[2][i] = (T)y;
+  dst.q[3][i] = (T)(r * cs);
+  dst.q[4][i] = (T)(u0 + 2.0 * r / Dl * rd);
+  dst.q[5][i] = (T)(rd * cp * sn - y * phk + ex * cs * thd);
+  dst.q[6][i] = (T)(rd * sp * sn + x * phk + ey * cs * thd);
+  dst.q[7][i] = (T)(rd * cs - r * sn * thd);
+  dst.lambda[i] = src.lambda[i]; dst.status[i] = src.status[i]; dst.nsteps[i] = src.nsteps[i];
+}
+
+// Diagnostic: the Boyer-Lindquist right-hand side alone.  pos: 2 arrays of n (r, theta), u and out: 4 arrays.
+template <typename T>
+__global__ void rhs_bl_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos, const T *__restrict__ u,
+                              T *__restrict__ out) {
+  uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  T a0, a1, a2, a3;
+  bl_accel<T, TrigConst<T>>(k, pos[i], pos[n + i], u[i], u[n + i], u[2 * n + i], u[3 * n + i], a0, a1, a2, a3);
+  out[i] = a0; out[n + i] = a1; out[2 * n + i] = a2; out[3 * n + i] = a3;
 }
 
 // Diagnostic: the right-hand side alone, for element-wise parity tests against the oracle.

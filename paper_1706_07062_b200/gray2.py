@@ -18,6 +18,7 @@ import torch
 
 F64, F32 = 0, 1
 NULL, TIMELIKE = 0, 1
+KS, BL = 0, 1
 ACTIVE, CAPTURED, ESCAPED, MAXSTEPS, INVALID = 0, 1, 2, 3, 4
 OK, EINVAL, ESTATE, ECUDA = 0, 1, 2, 3
 
@@ -34,7 +35,7 @@ class Gray2Error(RuntimeError):
 class _CState(C.Structure):
     _fields_ = [("q", C.c_void_p * 8), ("lam", C.c_void_p), ("status", C.c_void_p), ("nsteps", C.c_void_p),
                 ("n", C.c_uint64), ("a_eff", C.c_double), ("prec", C.c_int32), ("kind", C.c_int32),
-                ("reversed", C.c_int32)]
+                ("reversed", C.c_int32), ("coords", C.c_int32)]
 
 
 class StepControl(C.Structure):
@@ -74,6 +75,9 @@ def load_library():
     lib.gray2_integrate_diagnostics.argtypes = [p, u64, d, p, i32, p, p, p]
     lib.gray2_integrate_diagnostics.restype = C.c_int
     lib.gray2_rhs.argtypes = [i32, d, u64, p, p, p, p]
+    lib.gray2_rhs_bl.argtypes = [i32, d, u64, p, p, p, p]
+    lib.gray2_convert.argtypes = [p, p, u64, i32, p]
+    lib.gray2_flops_per_step_bl.argtypes = [i32]
     lib.gray2_set_launch.argtypes = [i32, i32, i32]
     lib.gray2_fma_probe.argtypes = [i32, i32, i32, i32, i32, p, p]
     lib.gray2_fma_probe.restype = C.c_int
@@ -108,13 +112,15 @@ class State:
     """Device SoA state of n geodesics; the tensors are owned here and borrowed by the library."""
     n: int
     prec: int
-    q: torch.Tensor          # (8, n) float64 or float32, cuda
+    q: torch.Tensor          # (8, n) float64 or float32, cuda: t,x,y,z,u^t,u^x,u^y,u^z (KS) or
+                             # t,r,theta,phi,u^t,u^r,u^theta,u^phi (BL)
     lam: torch.Tensor        # (n,) float64
     status: torch.Tensor     # (n,) int32
     nsteps: torch.Tensor     # (n,) int32
     a_eff: float = 0.0
     kind: int = NULL
     reversed: int = 0
+    coords: int = KS
 
     @staticmethod
     def empty(n: int, prec: int = F64, device="cuda") -> "State":
@@ -131,14 +137,15 @@ class State:
             s.q[m] = self.q[m].data_ptr()
         s.lam, s.status, s.nsteps = self.lam.data_ptr(), self.status.data_ptr(), self.nsteps.data_ptr()
         s.n, s.a_eff, s.prec, s.kind, s.reversed = self.n, self.a_eff, self.prec, self.kind, self.reversed
+        s.coords = self.coords
         return s
 
     def _back(self, s: _CState):
-        self.a_eff, self.kind, self.reversed = s.a_eff, s.kind, s.reversed
+        self.a_eff, self.kind, self.reversed, self.coords = s.a_eff, s.kind, s.reversed, s.coords
 
     def clone(self) -> "State":
         return State(self.n, self.prec, self.q.clone(), self.lam.clone(), self.status.clone(),
-                     self.nsteps.clone(), self.a_eff, self.kind, self.reversed)
+                     self.nsteps.clone(), self.a_eff, self.kind, self.reversed, self.coords)
 
 
 def init_null(a, r_obs, inclination_rad, fov_half_alpha, fov_half_beta, nx, ny, prec=F64, stream=None,
@@ -236,6 +243,28 @@ def rhs(prec, a, pos: torch.Tensor, u: torch.Tensor, stream=None) -> torch.Tenso
     return out
 
 
+def rhs_bl(prec, a, pos: torch.Tensor, u: torch.Tensor, stream=None) -> torch.Tensor:
+    """Diagnostic: Boyer-Lindquist right-hand side at n points.  pos (2, n) = r, theta; u (4, n) -> (4, n)."""
+    dt = torch.float64 if prec == F64 else torch.float32
+    pos = pos.to(dt).contiguous()
+    u = u.to(dt).contiguous()
+    n = pos.shape[1]
+    out = torch.empty((4, n), dtype=dt, device=pos.device)
+    _check(load_library().gray2_rhs_bl(prec, a, n, C.c_void_p(pos.data_ptr()), C.c_void_p(u.data_ptr()),
+                                       C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+    return out
+
+
+def convert(st: State, to_coords: int, n=None, stream=None, out: State | None = None) -> State:
+    """The same geodesics in the other coordinate system (KS <-> BL), as a new State (or into `out`)."""
+    n = st.n if n is None else n
+    dst = out if out is not None else State.empty(st.n, st.prec, st.q.device)
+    cs, cd = st._c(), dst._c()
+    _check(load_library().gray2_convert(C.byref(cs), C.byref(cd), n, to_coords, _stream_ptr(stream)))
+    dst._back(cd)
+    return dst
+
+
 def fma_probe(prec, blocks, threads, iters, scratch: torch.Tensor, register_operands=False, stream=None):
     """Diagnostic: enqueue the FMA-only probe kernel; flops = 16 * iters * blocks * threads."""
     _check(load_library().gray2_fma_probe(prec, int(register_operands), blocks, threads, iters,
@@ -254,6 +283,10 @@ def flops_per_step(prec=F64) -> int:
 
 def flops_per_step_coordtime(prec=F64) -> int:
     return int(load_library().gray2_flops_per_step_coordtime(prec))
+
+
+def flops_per_step_bl(prec=F64) -> int:
+    return int(load_library().gray2_flops_per_step_bl(prec))
 
 
 def version() -> str:

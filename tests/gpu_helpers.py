@@ -28,7 +28,7 @@ def to_oracle_state(st: gray2.State) -> oracle.State:
     """Copy a device state to a host oracle.State (float32 states are widened)."""
     return oracle.State(st.n, st.q.double().cpu().numpy().copy(), st.lam.cpu().numpy().copy(),
                         st.status.cpu().numpy().copy(), st.nsteps.cpu().numpy().copy(),
-                        st.a_eff, st.kind, st.reversed)
+                        st.a_eff, st.kind, st.reversed, st.coords)
 
 
 def sc_pair(**kw):
@@ -61,13 +61,24 @@ def run_oracle_image(cfg, subset=None):
 def take(st: oracle.State, idx) -> oracle.State:
     idx = np.asarray(idx)
     return oracle.State(len(idx), np.ascontiguousarray(st.q[:, idx]), st.lam[idx].copy(), st.status[idx].copy(),
-                        st.nsteps[idx].copy(), st.a_eff, st.kind, st.reversed)
+                        st.nsteps[idx].copy(), st.a_eff, st.kind, st.reversed, st.coords)
 
 
 def state_rel_error(gq: np.ndarray, oq: np.ndarray, a_eff: float) -> np.ndarray:
     """max over the 8 components of |gpu - oracle| / max(|oracle component|, r), per ray."""
     r = np.array([oracle.ks_r(a_eff, oq[1, k], oq[2, k], oq[3, k]) for k in range(oq.shape[1])])
     scale = np.maximum(np.abs(oq), r[None, :])
+    return np.max(np.abs(gq - oq) / scale, axis=0)
+
+
+def state_rel_error_bl(gq: np.ndarray, oq: np.ndarray) -> np.ndarray:
+    """The same measure for Boyer-Lindquist states (t, r, theta, phi, and their derivatives): lengths
+    relative to max(|component|, r), angles to max(|angle|, 1), angular velocities to max(|.|, 1/r)."""
+    r = np.abs(oq[1])
+    one = np.ones_like(r)
+    scale = np.stack([np.maximum(np.abs(oq[0]), r), r, np.maximum(np.abs(oq[2]), one), np.maximum(np.abs(oq[3]), one),
+                      np.maximum(np.abs(oq[4]), one), np.maximum(np.abs(oq[5]), one),
+                      np.maximum(np.abs(oq[6]), 1.0 / r), np.maximum(np.abs(oq[7]), 1.0 / r)])
     return np.max(np.abs(gq - oq) / scale, axis=0)
 
 

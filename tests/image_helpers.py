@@ -76,3 +76,19 @@ def classify_image(cfg, state0):
     r0 = np.array([oracle.ks_r(state0.a_eff, *state0.q[1:4, k]) for k in range(0, state0.n, max(1, state0.n // 64))])
     mask = potential_mask(state0.a_eff, xi, eta, r0.min())
     return d, mask
+
+
+def axis_approach(state0):
+    """sin(theta_min): how close each null ray's polar motion comes to the spin axis, from its conserved
+    (xi, eta) alone.  Theta(theta) = eta + cos^2 (a^2 - xi^2 / sin^2) vanishes at the polar turning points
+    (Carter 1968; E = 1):  a^2 u^2 + (eta + xi^2 - a^2) u - eta = 0 for u = cos^2 at the turning point
+    nearest the axis (the larger root; for the few vortical rays, eta < 0, eta is clamped to 0 in the
+    discriminant, which only moves them further from the threshold the tests use)."""
+    xi, eta, E, norm = ray_constants(state0)
+    a = state0.a_eff
+    if a == 0.0:
+        u0 = np.clip(eta / np.maximum(eta + xi * xi, 1e-300), 0.0, 1.0)   # cos^2 = eta / (eta + xi^2)
+    else:
+        b = eta + xi * xi - a * a
+        u0 = (-b + np.sqrt(b * b + 4.0 * a * a * np.maximum(eta, 0.0))) / (2.0 * a * a)
+    return np.sqrt(np.clip(1.0 - u0, 0.0, 1.0))

@@ -170,11 +170,15 @@ def test_convert_whole_state_and_argument_checks():
 
 # ---- the driver loop in BL coordinates ------------------------------------------------------------
 
-# Steps must not straddle Delta = 0, where eq. (1) is singular ("coordinate singularities at
-# the event horizons"): with h = eta r and |dr/dlambda| up to ~3 near the horizon, the capture radius needs
-# a margin of ~3 eta.  Every BL run of the suite uses capture_factor = 1.03 (DESIGN R20); the KS run it is
-# compared with uses the same value, so that step counts are comparable.
-BL_CAPTURE = 1.03
+# Eq. (1) is singular at Delta = 0 ("coordinate singularities at the event horizons") and, with
+# h = eta r, a ray that falls in reaches the horizon within one step of r = 1.01 r_+: on BL states the capture
+# test is therefore applied to the RK4 stage positions too (DESIGN R20), and the ordinary capture_factor works.
+BL_CAPTURE = 1.01
+# The other singularity of eq. (1), the axis, is left as it is: with h = eta r a passage
+# closer to the axis than about 2 eta radians cannot be resolved (the polar angle moves by ~eta per step), and
+# those rays come out wrong in BL -- the paper's reason for Kerr-Schild coordinates.  The BL comparisons below
+# are made on the rays whose polar turning point stays sin(theta_min) >= AXIS_MARGIN = 5 eta away (DESIGN R21).
+AXIS_MARGIN = 0.05
 
 
 def run_image(cfg, coords, eta=None, lambda_end=float("inf"), r_escape=None):
@@ -194,13 +198,16 @@ def test_bl_image_agrees_with_ks_image_and_with_carters_potential(cfg):
     k0, k1, kstats = run_image(cfg, oracle.KS)
     b0, b1, bstats = run_image(cfg, oracle.BL)
     d, mask = ih.classify_image(cfg, k0)
-    outside = d > 1e-3
-    assert outside.mean() > 0.98
+    outside = (d > 1e-3) & (ih.axis_approach(k0) >= AXIS_MARGIN)
+    assert outside.mean() > 0.9
     assert np.array_equal(b1.status[outside], k1.status[outside])
     assert np.array_equal((b1.status == oracle.CAPTURED)[outside], mask[outside])
-    assert bstats["n_invalid"] == 0 and bstats["n_active"] == 0 and bstats["n_maxsteps"] == 0
+    assert bstats["n_active"] == 0
     # the same geodesics, the same step rule h = eta r: step counts differ by truncation error only
-    assert np.max(np.abs(b1.nsteps - k1.nsteps)[outside]) <= 1
+    # (captured rays end a few steps earlier in BL, at the last step that stays outside the capture radius)
+    esc_k = outside & (k1.status == oracle.ESCAPED)
+    assert np.max(np.abs(b1.nsteps - k1.nsteps)[esc_k]) <= 1
+    assert np.all((k1.nsteps - b1.nsteps)[outside & ~esc_k] >= 0) and np.max((k1.nsteps - b1.nsteps)[outside]) <= 12
     # constants of motion are kept to the accuracy of the scheme in either system
     esc = outside & (b1.status == oracle.ESCAPED)
     # (rays that pass close to the axis lose accuracy in BL: hence median and maximum)
@@ -214,6 +221,60 @@ def test_bl_image_agrees_with_ks_image_and_with_carters_potential(cfg):
     er, eth = (np.abs(kb.q[1] - b1.q[1]) / kb.q[1])[same], np.abs(kb.q[2] - b1.q[2])[same]
     assert np.median(er) < 1e-6 and np.max(er) < 1e-2      # worst: strongly lensed rays near the axis (cfg2, i = 17 deg)
     assert np.median(eth) < 1e-7 and np.max(eth) < 1e-3
+
+
+def test_guarded_step_is_the_plain_step_unless_a_stage_is_inside_the_capture_radius():
+    a = 0.9
+    y = np.array([0.0, 6.0, 1.2, 0.3, 1.3, -0.7, 0.02, 0.05])      # moving inward at 0.7
+    h = 0.06                                                        # stages 2, 3 near r = 5.979, stage 4 near 5.958
+    plain = oracle.bl_rk4_step(a, y, h)
+    assert 5.955 < plain[1] < 5.961
+    hit, y1 = oracle.bl_rk4_step_guarded(a, y, h, 5.95)
+    assert not hit and np.array_equal(y1, plain)
+    hit, y1 = oracle.bl_rk4_step_guarded(a, y, h, 5.97)             # the full-step stage and the result are inside
+    assert hit and np.array_equal(y1, y)
+    hit, y1 = oracle.bl_rk4_step_guarded(a, y, h, plain[1] + 1e-9)  # the result alone decides as well
+    assert hit and np.array_equal(y1, y)
+    hit, y1 = oracle.bl_rk4_step_guarded(a, y, h, 5.99)             # already the first half-step stage
+    assert hit and np.array_equal(y1, y)
+
+
+@pytest.mark.parametrize("cfg", [inputs.CFG2_NULL.scaled(96, 80), inputs.CFG3_NULL.scaled(64, 64),
+                                 inputs.NullImageConfig("extremal", 1.0, 1000.0, 85.0, 8.0, 48, 48)], ids=lambda c: c.name)
+def test_no_ray_crosses_the_horizon_singularity(cfg):
+    """Every ray Carter's potential sends into the hole ends CAPTURED, none is thrown out by a stage evaluated
+    at Delta <= 0 (what happens without the stage test: a dozen rays of this very cfg2 image "escape")."""
+    b0, b1, stats = run_image(cfg, oracle.BL)
+    k0 = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    away = ih.axis_approach(k0) >= AXIS_MARGIN
+    if abs(cfg.a) < 1.0:
+        d, mask = ih.classify_image(cfg, k0)
+        outside = (d > 1e-3) & away
+        assert np.array_equal((b1.status == oracle.CAPTURED)[outside], mask[outside])
+    else:
+        _, k1, _ = run_image(cfg, oracle.KS)
+        assert (b1.status != k1.status)[away].mean() < 2e-3
+    cap = away & (b1.status == oracle.CAPTURED)
+    assert cap.sum() > 50
+    # stored at the last state outside the capture radius, at most about one step away from it
+    assert (b1.q[1][cap] >= BL_CAPTURE * cf.r_plus(cfg.a)).all() and (b1.q[1][cap] < 1.15 * cf.r_plus(cfg.a)).all()
+    assert np.all(np.isfinite(b1.q[:, away]))
+
+
+def test_rays_that_graze_the_axis_are_lost_in_bl_and_only_those():
+    """PAPER.md:49-51 made quantitative: in the cfg2 image (i = 17 deg) about a hundred of 7680 rays come out
+    with the wrong fate or step count in BL; every one of them passes within 0.025 rad of the axis; the
+    Kerr-Schild run of the same rays agrees with Carter's potential everywhere outside the critical band."""
+    cfg = inputs.CFG2_NULL.scaled(96, 80)
+    k0, k1, _ = run_image(cfg, oracle.KS)
+    b0, b1, _ = run_image(cfg, oracle.BL)
+    d, mask = ih.classify_image(cfg, k0)
+    outside = d > 1e-3
+    assert np.array_equal((k1.status == oracle.CAPTURED)[outside], mask[outside])
+    esc = k1.status == oracle.ESCAPED        # (captured rays stop a few steps earlier in BL: the stage test)
+    lost = outside & ((b1.status != k1.status) | (esc & (np.abs(b1.nsteps - k1.nsteps) > 1)))
+    assert 20 < lost.sum() < 400
+    assert ih.axis_approach(k0)[lost].max() < 0.025
 
 
 def test_bl_driver_is_fourth_order():
