@@ -36,9 +36,11 @@ INF = float("inf")
 FP_LANES = {"f64": 64, "f32": 128}
 
 # DRAM traffic of the dominant kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch, from the
-# `ncu --set full` captures summarised in profiles/r01_ncu_integrate_f{64,32}_v3.txt (cfg3, affine form).
+# `ncu --set full` captures summarised in profiles/r01_ncu_integrate_f{64,32}_v3.txt (cfg3, affine form) and
+# profiles/r01_ncu_integrate_bl_f{64,32}.txt (cfg3, Boyer-Lindquist form).
 # Algorithmic state traffic is 2 x 80 B (FP64) or 2 x 48 B (FP32) per ray.
-NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83903744 + 31966464, ("cfg3", "f32", "affine"): 50362880 + 1761536}
+NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83903744 + 31966464, ("cfg3", "f32", "affine"): 50362880 + 1761536,
+                  ("cfg3", "f64", "bl"): 84328448 + 31719936, ("cfg3", "f32", "bl"): 50350336 + 1810176}
 
 
 def nominal_peak_tflops(dtype: str, n_sms: int, sm_max_mhz: float) -> float:
@@ -350,7 +352,7 @@ def run_gpu(args):
                              ", coordinate time" if coord else ", Boyer-Lindquist" if bl else ("" if prec == gray2.F64 else "affine")),
                          "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": NCU_DRAM_BYTES.get((args.workload, args.dtype, args.form)),
-                         "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_integrate_*_v3.txt)",
+                         "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_integrate_*.txt)",
                          "flops_per_rk4_step": flops_per_step,
                          "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,
                          "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (n_sms, FP_LANES[args.dtype], sm_max_mhz),

@@ -15,10 +15,13 @@
 // Four reciprocals (Sigma, Delta, P, sin^2) and sin/cos of theta per evaluation: the trigonometric functions
 // are what the paper names as the cost of this system in double precision.
 //
-// sin and cos.  Only sin^2, cos^2 and sin cos enter, all of period pi: theta is reduced to |y| <= pi/2 by
-// y = theta - n pi (two-constant Cody-Waite with FMA, n by the add-and-subtract-2^52 trick), and sin y,
-// cos y are their Taylor polynomials in y^2 (remainder below 1e-18 in double with 10 / 11 terms, below
-// 1e-9 in float with 6 / 6): no quadrant logic, no table, no slow path, the same code for the packed type.
+// sin and cos.  Only sin^2 and sin cos enter (cos^2 = 1 - sin^2 inside Sigma), both of period pi, computed
+// without table or slow path from the Taylor polynomials of sin y, cos y in y^2:
+//   float / packed pair: y = theta - n pi, |y| <= pi/2 (two-constant Cody-Waite with FMA, n by the
+//     add-and-subtract-1.5*2^23 trick), 6 / 6 terms (remainder < 1e-9), no quadrant logic;
+//   double: y = theta - n pi/2, |y| <= pi/4, 8 / 8 terms (remainder < 2e-18) and a swap (sin, cos) ->
+//     (cos, -sin) for odd n; the selects run on the integer pipe, which is idle in the FP64 kernel, and save
+//     six FP64-pipe instructions per evaluation over the period-pi form (10 / 11 terms).
 #pragma once
 #include "ks_geodesic.cuh"
 
@@ -26,14 +29,16 @@ namespace gray2 {
 
 template <typename T> struct TrigConst;
 template <> struct TrigConst<double> {
-  static constexpr int NS = 10, NC = 11;
-  static constexpr double inv_pi = 0.31830988618379067154, magic = 6755399441055744.0;   // 1.5 * 2^52
-  static constexpr double pi_hi = 3.14159265358979311600, pi_lo = 1.2246467991473532e-16;
+  static constexpr int NS = 8, NC = 8;
+  static constexpr bool quadrant = true;
+  static constexpr double inv_period = 0.63661977236758134308, magic = 6755399441055744.0;   // 2/pi, 1.5 * 2^52
+  static constexpr double p_hi = 1.57079632679489655800, p_lo = 6.123233995736766e-17;       // pi/2 = p_hi + p_lo
 };
 template <> struct TrigConst<float> {
   static constexpr int NS = 6, NC = 6;
-  static constexpr double inv_pi = 0.31830988618379067154, magic = 12582912.0;             // 1.5 * 2^23
-  static constexpr double pi_hi = 3.1415927410125732, pi_lo = -8.742278000372485e-8;       // float(pi), pi - float(pi)
+  static constexpr bool quadrant = false;
+  static constexpr double inv_period = 0.31830988618379067154, magic = 12582912.0;           // 1/pi, 1.5 * 2^23
+  static constexpr double p_hi = 3.1415927410125732, p_lo = -8.742278000372485e-8;           // float(pi), pi - float(pi)
 };
 
 // S(z) = sum_{k>=1} (-1)^k z^(k-1) / (2k+1)!  so that  sin y = y + y^3 S(y^2)
@@ -59,27 +64,35 @@ template <typename T, int N> __device__ __forceinline__ T cos_series(T z) {
   return p;
 }
 
-// K = TrigConst of the scalar type behind T (float for the packed pair).
+// sin^2(theta) and sin(theta) cos(theta).  K = TrigConst of the scalar type behind T (float for the pair).
 template <typename T, typename K>
-__device__ __forceinline__ void bl_trig(T th, T &s2, T &c2, T &sc) {
-  T n = (th * T(K::inv_pi) + T(K::magic)) + T(-K::magic);      // nearest integer to theta / pi
-  T y = fma_(n, T(-K::pi_hi), th);
-  y = fma_(n, T(-K::pi_lo), y);
+__device__ __forceinline__ void bl_trig(T th, T &s2, T &sc) {
+  T t = th * T(K::inv_period) + T(K::magic);       // the integer nearest to theta / period, in the low bits
+  T n = t + T(-K::magic);
+  T y = fma_(n, T(-K::p_hi), th);
+  y = fma_(n, T(-K::p_lo), y);
   T z = y * y;
   T s = fma_(y * z, sin_series<T, K::NS>(z), y);
   T c = fma_(z, cos_series<T, K::NC>(z), T(1));
-  s2 = s * s; c2 = c * c; sc = s * c;
+  if constexpr (K::quadrant) {
+    // period pi/2: odd n  ->  (sin, cos)(theta) = +-(cos y, -sin y)
+    const bool odd = (__double2loint(t) & 1) != 0;
+    const T ss = odd ? c : s;
+    const T cc = odd ? -s : c;
+    s = ss; c = cc;
+  }
+  s2 = s * s; sc = s * c;
 }
 
 // xddot^mu at (r, theta) for xdot = (u0, u1, u2, u3) = d(t, r, theta, phi)/dlambda.
 template <typename T, typename K>
 __device__ __forceinline__ void bl_accel(const SpinConst<T> &k, T r, T th, T u0, T u1, T u2, T u3,
                                          T &a0, T &a1, T &a2, T &a3) {
-  T s2, c2, sc;
-  bl_trig<T, K>(th, s2, c2, sc);
+  T s2, sc;
+  bl_trig<T, K>(th, s2, sc);
   const T r2 = r * r;
-  const T Sig = fma_(k.a2, c2, r2);
   const T P = r2 + k.a2;
+  const T Sig = fma_(-k.a2, s2, P);               // r^2 + a^2 cos^2
   const T tr = r + r;
   const T Dl = P + (-tr);
   const T iS = fastmath<T>::rcp(Sig), iD = fastmath<T>::rcp(Dl), iP = fastmath<T>::rcp(P), is2 = fastmath<T>::rcp(s2);

@@ -134,14 +134,22 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
   *found = true;
   if constexpr (sizeof(T) == 8) {
     if (form == 1) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, st);
-    if (form == 2) return launch_integrate<T, 128, 3, 2>(s, n, p, q, steps, st);
+    if (form == 2) {
+      if (threads == 128 && blocks == 4) return launch_integrate<T, 128, 4, 2>(s, n, p, q, steps, st);
+      if (threads == 64 && blocks == 6) return launch_integrate<T, 64, 6, 2>(s, n, p, q, steps, st);
+      return launch_integrate<T, 128, 3, 2>(s, n, p, q, steps, st);
+    }
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
     GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(128, 2)
 #undef GRAY2_VARIANT
   } else {
     if (form == 1) return launch_integrate_x2<256, 2, 1>(s, n, p, q, steps, st);
-    if (form == 2) return launch_integrate_x2<256, 2, 2>(s, n, p, q, steps, st);
+    if (form == 2) {
+      if (threads == 128 && blocks == 4) return launch_integrate_x2<128, 4, 2>(s, n, p, q, steps, st);
+      if (threads == 128 && blocks == 3) return launch_integrate_x2<128, 3, 2>(s, n, p, q, steps, st);
+      return launch_integrate_x2<256, 2, 2>(s, n, p, q, steps, st);
+    }
 #define GRAY2_VARIANT_X2(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, st);
 #define GRAY2_VARIANT(TH, BL) \
@@ -450,11 +458,11 @@ int gray2_flops_per_step(int32_t prec) { (void)prec; return 558; }
 int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 562; }
 
 /* Boyer-Lindquist form, source-level count of bl_geodesic.cuh (same conventions):
- *   sin^2, cos^2, sin cos of theta: reduction 8, series 21 + 22, products 3 -> 54 (double: 10 / 11 terms),
- *                                   36 (float: 6 / 6 terms)
- *   rest of the right-hand side 87 (4 of them reciprocals)  ->  141 / 123 per right-hand side
- *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 666 / 594 per step. */
-int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 594 : 666; }
+ *   sin^2 and sin cos of theta: reduction 8, series 17 + 16, products 2 -> 43 (double: 8 / 8 terms, period pi/2),
+ *                               reduction 8, series 13 + 12, products 2 -> 35 (float: 6 / 6 terms, period pi)
+ *   rest of the right-hand side 87 (4 of them reciprocals)  ->  130 / 122 per right-hand side
+ *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 622 / 590 per step. */
+int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 590 : 622; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
