@@ -8,7 +8,8 @@ A "step" is one pass of the whole path over one batch: gray2_init_null (image-pl
 -> gray2_integrate (fused RHS + RK4 + termination + refill) -> gray2_invariants, on the 1024 x 1024
 Kerr image of BASELINE.json configs[2] ("cfg3": a = 0.9375, r_obs = 1000 M, i = 60 deg, +-15 M), which is
 the workload north_star quotes the target on.  The metric is geodesic RK4 steps per second (whole job,
-summed over ranks; each rank traces its own image: weak scaling, no collective on the data path).
+summed over ranks; each rank traces its own image: weak scaling, no collective on the data path;
+--scaling strong shares ONE image among the ranks in tiles of 4096 rays, again without a collective).
 
 One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every field.
 """
@@ -29,6 +30,7 @@ if ROOT not in sys.path:
 
 METRIC = "geodesic RK4 steps/sec on 1 B200 (FP64, FP32) and fraction of non-tensor FP peak"
 UNIT = "RK4 steps/s"
+SHARD_TILE = 4096          # rays per tile when one image is shared by several GPUs (--scaling strong)
 INF = float("inf")
 
 # Non-tensor FP peak of a B200 from unit counts and clocks: 148 SMs x 64 FP64 lanes
@@ -206,15 +208,23 @@ def run_gpu(args):
 
     sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
                             capture_factor=cfg.capture_factor)
-    st = gray2.State.empty(cfg.n, prec)
-    st_ks = gray2.State.empty(cfg.n, prec) if bl else st
+    # --scaling strong: ONE image shared by all ranks, rays dealt out in tiles of 4096;
+    # weak (default): every rank traces its own image.  Neither has a collective on the data path.
+    strong = args.scaling == "strong" and world > 1
+    n_local = gray2.shard_count(cfg.n, SHARD_TILE, rank, world) if strong else cfg.n
+    st = gray2.State.empty(n_local, prec)
+    st_ks = gray2.State.empty(n_local, prec) if bl else st
     stats = gray2.new_stats()
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     def one_step(ev=None):
         if ev: ev[0].record(stream)
-        gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st_ks)
+        if strong:
+            gray2.init_null_shard(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, SHARD_TILE,
+                                  rank, world, prec=prec, out=st_ks)
+        else:
+            gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st_ks)
         if bl: gray2.convert(st_ks, gray2.BL, out=st)
         if ev: ev[1].record(stream)
         integrate(st, INF, sc, stats=stats)
@@ -253,8 +263,12 @@ def run_gpu(args):
     clocks = sampler.stop(t_window0, time.perf_counter())
 
     # ---- end to end through the public API with HOST buffers (pinned): H2D of the 8-vectors, D2H of results
-    host_in = torch.empty((cfg.n, 8), dtype=torch.float64).pin_memory()
-    src = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=gray2.F64)
+    host_in = torch.empty((n_local, 8), dtype=torch.float64).pin_memory()
+    if strong:
+        src = gray2.init_null_shard(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, SHARD_TILE,
+                                    rank, world, prec=gray2.F64)
+    else:
+        src = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=gray2.F64)
     host_in.copy_(src.q.t())          # outside the timed region: the user's 8-vectors, resident in host memory
     a_eff = src.a_eff
     del src
@@ -263,7 +277,7 @@ def run_gpu(args):
     # Each chunk has its own contiguous device state and pinned host result buffers, so every copy is a
     # plain asynchronous memcpy.
     n_chunks = max(1, args.e2e_chunks)
-    bounds = [(cfg.n * c // n_chunks, cfg.n * (c + 1) // n_chunks) for c in range(n_chunks)]
+    bounds = [(n_local * c // n_chunks, n_local * (c + 1) // n_chunks) for c in range(n_chunks)]
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
     host_in_np = host_in.numpy()
     parts, parts_ks, host_out, chunk_stats = [], [], [], []
@@ -338,11 +352,12 @@ def run_gpu(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_step / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": cfg.name, "rays_per_gpu": cfg.n, "rk4_steps_per_pass": steps_total // args.steps,
+            "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": cfg.name, "rays_per_gpu": n_local, "rk4_steps_per_pass": steps_total // args.steps,
                        "a": cfg.a, "r_obs": cfg.r_obs, "inclination_deg": cfg.inclination_deg, "fov_half": cfg.fov,
                        "form": args.form, "step_rule": ("dt = %g r" if coord else "dlambda = %g r") % cfg.eta, "l2": "flushed between timed iterations (256 MiB fill)",
-                       "parallelism": "independent image per GPU, no collective"},
+                       "parallelism": ("one image dealt out in tiles of %d rays, no collective" % SHARD_TILE) if strong
+                                      else "independent image per GPU, no collective"},
             "clocks": clocks,
             "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "gray2_init_timelike(host 8-vectors) -> %sgray2_integrate -> gray2_invariants -> D2H of state, invariants, stats" % ("gray2_convert -> " if bl else ""),
@@ -377,6 +392,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1 only. weak: one image per GPU; strong: one image shared by the GPUs (tiles of 4096 rays)")
     ap.add_argument("--form", default="affine", choices=["affine", "coordtime", "bl"],
                     help="affine: gray2_integrate (eq. 13-14); coordtime: gray2_integrate_coordtime (eq. 18); "
                          "bl: gray2_integrate on Boyer-Lindquist states (eq. 1; the paper's Table 2 BL rows)")

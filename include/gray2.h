@@ -93,6 +93,17 @@ typedef struct { uint64_t steps, n_captured, n_escaped, n_maxsteps, n_invalid, n
 int gray2_init_null(gray2_state *s, double a, double r_obs, double inclination_rad,
                     double fov_half_alpha, double fov_half_beta, int32_t nx, int32_t ny,
                     void *cuda_stream);
+/* One image shared by `world` GPUs (geodesics are independent, "trivially parallelizable";
+ * SURVEY 8(e)): the nx*ny ray indices are dealt out in tiles of tile_rays consecutive indices, tile t to rank
+ * t mod world, so that the long near-critical rays spread evenly over the GPUs.  Fills the rays of rank
+ * `rank`, compactly: shard-local ray j is the image's ray ((j / tile_rays) * world + rank) * tile_rays +
+ * j % tile_rays, with the same initial data, bit for bit, as gray2_init_null gives that ray.  s->n must equal
+ * gray2_shard_count(nx*ny, tile_rays, rank, world).  No data moves between GPUs during integration; the
+ * caller gathers the shards afterwards if it wants the image in one place. */
+int gray2_init_null_shard(gray2_state *s, double a, double r_obs, double inclination_rad,
+                          double fov_half_alpha, double fov_half_beta, int32_t nx, int32_t ny,
+                          uint64_t tile_rays, int32_t rank, int32_t world, void *cuda_stream);
+uint64_t gray2_shard_count(uint64_t n, uint64_t tile_rays, int32_t rank, int32_t world);   /* 0 on bad arguments */
 
 /* Explicit initial conditions.  host_xu8: HOST array of n x 8 doubles (AoS: t,x,y,z,u^t,u^x,u^y,u^z).
  * Copies them into the first n slots of the SoA state (converted to float for F32); with

@@ -249,25 +249,50 @@ extern "C" {
 const char *gray2_last_error(void) { return g_err; }
 const char *gray2_version(void) { return "gray2-b200 0.1 (sm_100a)"; }
 
-int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double Wa, double Wb,
-                    int32_t nx, int32_t ny, void *cuda_stream) {
+/* Number of rays of rank `rank` when n rays are dealt out in tiles of tile_rays, tile t to rank t mod world. */
+uint64_t gray2_shard_count(uint64_t n, uint64_t tile_rays, int32_t rank, int32_t world) {
+  if (tile_rays == 0 || world <= 0 || rank < 0 || rank >= world) return 0;
+  const uint64_t tiles = (n + tile_rays - 1) / tile_rays;                 // the last one may be ragged
+  const uint64_t mine = tiles / (uint64_t)world + ((uint64_t)rank < tiles % (uint64_t)world ? 1 : 0);
+  if (mine == 0) return 0;
+  const uint64_t last_tile = tiles - 1, last_size = n - last_tile * tile_rays;
+  const bool own_last = last_tile % (uint64_t)world == (uint64_t)rank;
+  return own_last ? (mine - 1) * tile_rays + last_size : mine * tile_rays;
+}
+
+int gray2_init_null_shard(gray2_state *s, double a, double r_obs, double inc, double Wa, double Wb,
+                          int32_t nx, int32_t ny, uint64_t tile_rays, int32_t rank, int32_t world,
+                          void *cuda_stream) {
   if (s) s->coords = GRAY2_KS;
   int rc = check_state(s, "gray2_init_null");
   if (rc) return rc;
   if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_null: |a| must be <= 1 (got %g)", a);
-  if (nx <= 0 || ny <= 0 || (uint64_t)nx * (uint64_t)ny != s->n)
-    return fail(GRAY2_EINVAL, "gray2_init_null: nx*ny (%d x %d) must equal s->n (%llu)", nx, ny, (unsigned long long)s->n);
+  if (nx <= 0 || ny <= 0) return fail(GRAY2_EINVAL, "gray2_init_null: nx and ny must be positive");
+  if (tile_rays == 0 || world <= 0 || rank < 0 || rank >= world)
+    return fail(GRAY2_EINVAL, "gray2_init_null_shard: need tile_rays > 0 and 0 <= rank < world");
+  const uint64_t n_local = gray2_shard_count((uint64_t)nx * (uint64_t)ny, tile_rays, rank, world);
+  if (n_local != s->n)
+    return fail(GRAY2_EINVAL, "gray2_init_null: s->n (%llu) must equal the number of rays of this call (%llu of %d x %d)",
+                (unsigned long long)s->n, (unsigned long long)n_local, nx, ny);
   if (!(r_obs > 1.0 + sqrt(1.0 - a * a))) return fail(GRAY2_EINVAL, "gray2_init_null: r_obs must exceed r_plus");
   if (!(Wa > 0.0) || !(Wb > 0.0) || !isfinite(inc)) return fail(GRAY2_EINVAL, "gray2_init_null: bad field of view or inclination");
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   s->a_eff = -a; s->kind = GRAY2_NULL; s->reversed = 1; s->coords = GRAY2_KS;
   unsigned grid = (unsigned)((s->n + 255) / 256);
   if (s->prec == GRAY2_F64)
-    gray2::init_null_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), -a, r_obs, sin(inc), cos(inc), Wa, Wb, nx, ny);
+    gray2::init_null_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), n_local, -a, r_obs, sin(inc), cos(inc), Wa, Wb,
+                                                          nx, ny, tile_rays, (uint32_t)rank, (uint32_t)world);
   else
-    gray2::init_null_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), -a, r_obs, sin(inc), cos(inc), Wa, Wb, nx, ny);
+    gray2::init_null_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), n_local, -a, r_obs, sin(inc), cos(inc), Wa, Wb,
+                                                         nx, ny, tile_rays, (uint32_t)rank, (uint32_t)world);
   CUDA_TRY(cudaGetLastError());
   return GRAY2_OK;
+}
+
+int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double Wa, double Wb,
+                    int32_t nx, int32_t ny, void *cuda_stream) {
+  if (nx <= 0 || ny <= 0) return fail(GRAY2_EINVAL, "gray2_init_null: nx and ny must be positive");
+  return gray2_init_null_shard(s, a, r_obs, inc, Wa, Wb, nx, ny, (uint64_t)nx * (uint64_t)ny, 0, 1, cuda_stream);
 }
 
 int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t renorm,

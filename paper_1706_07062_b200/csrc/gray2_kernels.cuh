@@ -51,12 +51,18 @@ __device__ __forceinline__ double solve_ut(double a, double x, double y, double 
   return (B + sqrt(B * B + A * C)) / A;
 }
 
+// Shard of one image: ray indices are dealt out in tiles of `tile` consecutive indices, tile t
+// to rank t mod world; the shard-local ray `idx` of rank `rank` is the image's ray
+//   pix = ((idx / tile) * world + rank) * tile + idx % tile.
+// The whole image is the case tile = nx*ny, rank = 0, world = 1 (pix = idx).
 template <typename T>
-__global__ void init_null_kernel(StateView<T> s, double a_eff, double r_obs, double sin_i, double cos_i,
-                                 double Wa, double Wb, int32_t nx, int32_t ny) {
-  int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (int64_t)nx * ny) return;
-  int32_t j = (int32_t)(idx % nx), kk = (int32_t)(idx / nx);
+__global__ void init_null_kernel(StateView<T> s, uint64_t n_local, double a_eff, double r_obs, double sin_i,
+                                 double cos_i, double Wa, double Wb, int32_t nx, int32_t ny, uint64_t tile,
+                                 uint32_t rank, uint32_t world) {
+  uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_local) return;
+  uint64_t pix = ((idx / tile) * world + rank) * tile + idx % tile;
+  int32_t j = (int32_t)(pix % (uint64_t)nx), kk = (int32_t)(pix / (uint64_t)nx);
   double alpha = -Wa + ((double)j + 0.5) * (2.0 * Wa / (double)nx);
   double beta = -Wb + ((double)kk + 0.5) * (2.0 * Wb / (double)ny);
   // n = (sin i, 0, cos i), e_alpha = (0,1,0), e_beta = (-cos i, 0, sin i)

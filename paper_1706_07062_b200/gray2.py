@@ -66,6 +66,9 @@ def load_library():
     d, p, i32, u64 = C.c_double, C.c_void_p, C.c_int32, C.c_uint64
     lib.gray2_init_null.argtypes = [p, d, d, d, d, d, i32, i32, p]
     lib.gray2_init_timelike.argtypes = [p, d, p, u64, i32, p]
+    lib.gray2_init_null_shard.argtypes = [p, d, d, d, d, d, i32, i32, u64, i32, i32, p]
+    lib.gray2_shard_count.argtypes = [u64, u64, i32, i32]
+    lib.gray2_shard_count.restype = u64
     lib.gray2_integrate.argtypes = [p, u64, d, p, i32, p, p]
     lib.gray2_integrate_coordtime.argtypes = [p, u64, d, p, i32, p, p]
     lib.gray2_integrate_coordtime.restype = C.c_int
@@ -154,6 +157,21 @@ def init_null(a, r_obs, inclination_rad, fov_half_alpha, fov_half_beta, nx, ny, 
     cs = st._c()
     _check(load_library().gray2_init_null(C.byref(cs), a, r_obs, inclination_rad, fov_half_alpha,
                                           fov_half_beta, nx, ny, _stream_ptr(stream)))
+    st._back(cs)
+    return st
+
+
+def shard_count(n, tile_rays, rank, world) -> int:
+    return int(load_library().gray2_shard_count(n, tile_rays, rank, world))
+
+
+def init_null_shard(a, r_obs, inclination_rad, fov_half_alpha, fov_half_beta, nx, ny, tile_rays, rank, world,
+                    prec=F64, stream=None, out: State | None = None) -> State:
+    """This rank's rays of an image dealt out in tiles of tile_rays to `world` GPUs (see gray2.h)."""
+    st = out if out is not None else State.empty(shard_count(nx * ny, tile_rays, rank, world), prec)
+    cs = st._c()
+    _check(load_library().gray2_init_null_shard(C.byref(cs), a, r_obs, inclination_rad, fov_half_alpha,
+                                                fov_half_beta, nx, ny, tile_rays, rank, world, _stream_ptr(stream)))
     st._back(cs)
     return st
 

@@ -26,8 +26,16 @@ def _worker(rank, world, port, out):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     lo, hi = multi.shard_range(1001, rank, world)
     times, work = multi.reduce_job([1.0 + rank, 0.5], [hi - lo, 10 * (rank + 1)])
+    # one image dealt out in tiles: every rank holds values of its own rays only, in shard
+    # order; after the gather every rank holds the whole image in ray order
+    n, tile = 1003, 64                                    # 16 tiles, the last one ragged
+    mine = multi.shard_global_index(n, tile, rank, world)
+    local = torch.stack([mine.double() * 3.0 + 1.0, -mine.double()])       # (2, n_local): "results" of my rays
+    full = multi.gather_image(local, n, tile)
+    local_i = (mine % 5).to(torch.int32)                                     # a status-like integer array
+    full_i = multi.gather_image(local_i, n, tile)
     if rank == 0:
-        torch.save({"times": times, "work": work}, out)
+        torch.save({"times": times, "work": work, "full": full, "full_i": full_i, "n_local": mine.numel()}, out)
     dist.barrier()
     dist.destroy_process_group()
 
@@ -38,6 +46,10 @@ def test_two_rank_reduction_and_sharding(tmp_path):
     res = torch.load(out)
     assert res["times"] == [2.0, 0.5]          # max over ranks
     assert res["work"] == [1001.0, 30.0]       # sum over ranks: the shards tile the units exactly
+    g = torch.arange(1003, dtype=torch.float64)
+    assert torch.equal(res["full"], torch.stack([g * 3.0 + 1.0, -g]))
+    assert torch.equal(res["full_i"], (torch.arange(1003) % 5).to(torch.int32))
+    assert res["n_local"] == 8 * 64            # rank 0 owns tiles 0, 2, ..., 14 (the ragged tile 15 is rank 1's)
 
 
 def test_shard_range_tiles_exactly():
@@ -51,3 +63,21 @@ def test_shard_range_tiles_exactly():
             sizes = [hi - lo for lo, hi in pieces]
             assert max(sizes) - min(sizes) <= 1
     assert multi.reduce_job([3.0], [5]) == ([3.0], [5.0])    # single process: identity
+
+
+def test_tile_dealing_is_a_permutation_and_matches_the_library_count():
+    sys.path.insert(0, ROOT)
+    import ctypes as C
+    from paper_1706_07062_b200 import build, multi
+    lib = C.CDLL(build.build())
+    lib.gray2_shard_count.argtypes = [C.c_uint64, C.c_uint64, C.c_int32, C.c_int32]
+    lib.gray2_shard_count.restype = C.c_uint64
+    for n, tile, world in ((10, 3, 2), (4096, 4096, 3), (1000, 7, 3), (5, 10, 4), (1 << 20, 4096, 8), (77, 1, 5)):
+        parts = [multi.shard_global_index(n, tile, r, world) for r in range(world)]
+        assert sorted(torch.cat(parts).tolist()) == list(range(n))
+        for r, p in enumerate(parts):
+            assert lib.gray2_shard_count(n, tile, r, world) == p.numel()
+            # the formula of gray2_init_null_shard
+            j = torch.arange(p.numel())
+            assert torch.equal(p, ((j // tile) * world + r) * tile + j % tile)
+    assert lib.gray2_shard_count(10, 0, 0, 1) == 0 and lib.gray2_shard_count(10, 3, 2, 2) == 0    # bad arguments
