@@ -14,6 +14,10 @@
  *                        until it is close to the horizon, escapes, or exhausts its step budget
  *
  *   gray2_invariants     E, L_z, Carter Q and u.u ("u^2"; Table 1 "Phi", "Q")
+ * and, around these four: gray2_integrate_coordtime (the coordinate-time form),
+ * gray2_integrate_diagnostics (the convergence measurements of section 3), gray2_convert plus
+ * gray2_state.coords (the Boyer-Lindquist system of the paper's Table 2, behind the same gray2_integrate),
+ * gray2_init_null_shard (one image shared by several GPUs).
  *
  * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
  * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
