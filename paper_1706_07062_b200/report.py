@@ -174,9 +174,41 @@ def report_paper_benchmark():
     return out
 
 
+def report_bl_vs_ks():
+    """The same images traced in both coordinate systems (PAPER.md:49-51 made quantitative): how many rays
+    end with a different fate in Boyer-Lindquist coordinates, and where they are (all of them graze the
+    axis: |L_z|/E small), per image config, FP64.  Kerr-Schild is the reference: tests/ pin it to Carter's
+    potential on every ray outside the critical band."""
+    out = {}
+    for cfg in (inputs.CFG1_NULL, inputs.CFG2_NULL, inputs.CFG3_NULL, inputs.CFG5_NULL):
+        sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
+                                capture_factor=cfg.capture_factor)
+        ks = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+        E, Lz, Q, _ = gray2.invariants(ks)
+        bl = gray2.convert(ks, gray2.BL)
+        sk, sb = gray2.new_stats(), gray2.new_stats()
+        _, tk = _timed(lambda: gray2.integrate(ks, INF, sc, stats=sk))
+        _, tb = _timed(lambda: gray2.integrate(bl, INF, sc, stats=sb))
+        differ = ks.status != bl.status
+        esc = (ks.status == gray2.ESCAPED) & ~differ
+        late = esc & ((ks.nsteps - bl.nsteps).abs() > 1)
+        xi = (Lz / E).abs()
+        out[cfg.name] = {
+            "rays": cfg.n, "ks": gray2.stats_dict(sk), "bl": gray2.stats_dict(sb),
+            "ks_steps_per_s": gray2.stats_dict(sk)["steps"] / tk, "bl_steps_per_s": gray2.stats_dict(sb)["steps"] / tb,
+            "rays_with_different_fate": int(differ.sum()), "fraction": float(differ.float().mean()),
+            "escaped_rays_with_step_count_off_by_more_than_1": int(late.sum()),
+            "max_abs_Lz_over_E_of_those_rays": float(xi[differ | late].max()) if bool((differ | late).any()) else None,
+            "median_abs_Lz_over_E_of_all_rays": float(xi.median()),
+        }
+        del ks, bl
+        torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--configs", default="1,2,3,4,5", help="comma list of 1..5 and P (the paper's benchmark shape)")
+    ap.add_argument("--configs", default="1,2,3,4,5", help="comma list of 1..5, P (the paper's benchmark shape), B (Boyer-Lindquist vs Kerr-Schild images)")
     ap.add_argument("--cfg4-steps", type=int, default=100000)
     ap.add_argument("--cfg4-n", type=int, default=1 << 20)
     args = ap.parse_args()
@@ -196,6 +228,8 @@ def main():
         out["cfg5"]["f64"] = run_image(inputs.CFG5_NULL, gray2.F64)[1]
     if "P" in want:
         out["paper_benchmark"] = report_paper_benchmark()
+    if "B" in want:
+        out["bl_vs_ks"] = report_bl_vs_ks()
     print(json.dumps(out, indent=1))
 
 
