@@ -17,6 +17,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import subprocess
@@ -375,10 +376,14 @@ def run_gpu(args):
                          "fma_probe_register_operands_tflops": probe["regs"]},
         }
         if not args.no_cpu_baseline and world == 1:
-            v, s_per, cores, sub = time_oracle(cfg, args.oracle_side, 1, 0)
+            # a first pass on oracle_side^2 rays sizes the sample: about 12 s of wall clock on this box's cores
+            _, s_probe, _, _ = time_oracle(cfg, args.oracle_side, 1, 0)
+            side = int(args.oracle_side * math.sqrt(max(1.0, 12.0 / max(s_probe, 1e-3)))) // 32 * 32
+            side = max(args.oracle_side, min(side, 512, cfg.nx))
+            v, s_per, cores, sub = time_oracle(cfg, side, 1, 0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": "%s field of view on %dx%d rays, one pass (%.1f s)" % (
-                                        args.workload, args.oracle_side, args.oracle_side, s_per)}
+                                        args.workload, side, side, s_per)}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
