@@ -168,7 +168,7 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, cons
                    gray2_stats *device_stats, cudaStream_t st) {
   const double a = s->a_eff;
   gray2::StepParams<T> p;
-  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a);
+  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a); p.k.four_a2 = (T)(4.0 * a * a);
   p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
   p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
   p.r_escape = (T)sc->r_escape;
@@ -215,7 +215,7 @@ int diag_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_co
                      const gray2_diagnostics *d, gray2_stats *device_stats, cudaStream_t st) {
   const double a = s->a_eff;
   gray2::StepParams<T> p;
-  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a);
+  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a); p.k.four_a2 = (T)(4.0 * a * a);
   p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
   p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
   p.r_escape = (T)sc->r_escape;
@@ -448,10 +448,10 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   unsigned grid = (unsigned)((n + 127) / 128);
   if (prec == GRAY2_F64) {
-    gray2::SpinConst<double> k{a, a * a, 2.0 * a, 2.0 * a * a};
+    gray2::SpinConst<double> k{a, a * a, 2.0 * a, 2.0 * a * a, 4.0 * a * a};
     gray2::rhs_kernel<double><<<grid, 128, 0, st>>>(k, n, (const double *)pos, (const double *)u, (double *)out);
   } else {
-    gray2::SpinConst<float> k{(float)a, (float)(a * a), (float)(2.0 * a), (float)(2.0 * a * a)};
+    gray2::SpinConst<float> k{(float)a, (float)(a * a), (float)(2.0 * a), (float)(2.0 * a * a), (float)(4.0 * a * a)};
     gray2::rhs_kernel<float><<<grid, 128, 0, st>>>(k, n, (const float *)pos, (const float *)u, (float *)out);
   }
   CUDA_TRY(cudaGetLastError());
@@ -464,10 +464,10 @@ int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   unsigned grid = (unsigned)((n + 127) / 128);
   if (prec == GRAY2_F64) {
-    gray2::SpinConst<double> k{a, a * a, 2.0 * a, 2.0 * a * a};
+    gray2::SpinConst<double> k{a, a * a, 2.0 * a, 2.0 * a * a, 4.0 * a * a};
     gray2::rhs_bl_kernel<double><<<grid, 128, 0, st>>>(k, n, (const double *)pos, (const double *)u, (double *)out);
   } else {
-    gray2::SpinConst<float> k{(float)a, (float)(a * a), (float)(2.0 * a), (float)(2.0 * a * a)};
+    gray2::SpinConst<float> k{(float)a, (float)(a * a), (float)(2.0 * a), (float)(2.0 * a * a), (float)(4.0 * a * a)};
     gray2::rhs_bl_kernel<float><<<grid, 128, 0, st>>>(k, n, (const float *)pos, (const float *)u, (float *)out);
   }
   CUDA_TRY(cudaGetLastError());
@@ -475,12 +475,12 @@ int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void
 }
 
 /* Source-level count of ks_geodesic.cuh (FMA = 2, add/mul = 1, rsqrt/rcp = 1; negations and compares free):
- *   radius 16, rest of geometry 23, velocity part 75  ->  114 per right-hand side
- *   4 x 114 + RK4 combination 100 + step rule and lambda update 2 = 558 per step (both precisions). */
-int gray2_flops_per_step(int32_t prec) { (void)prec; return 558; }
+ *   radius 16, rest of geometry 19, velocity part 72  ->  107 per right-hand side
+ *   4 x 107 + RK4 combination 100 + step rule and lambda update 2 = 530 per step (both precisions). */
+int gray2_flops_per_step(int32_t prec) { (void)prec; return 530; }
 
-/* Coordinate-time form: 4 x (114 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
-int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 562; }
+/* Coordinate-time form: 4 x (107 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
+int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 534; }
 
 /* Boyer-Lindquist form, source-level count of bl_geodesic.cuh (same conventions):
  *   sin^2 and sin cos of theta: reduction 8, series 17 + 16, products 2 -> 43 (double: 8 / 8 terms, period pi/2),

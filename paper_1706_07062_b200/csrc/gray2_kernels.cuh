@@ -286,7 +286,7 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
                        unsigned long long *steps_out) {
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const SpinConst<f32x2> k{f32x2(p.k.a), f32x2(p.k.a2), f32x2(p.k.two_a), f32x2(p.k.two_a2)};
+  const SpinConst<f32x2> k{f32x2(p.k.a), f32x2(p.k.a2), f32x2(p.k.two_a), f32x2(p.k.two_a2), f32x2(p.k.four_a2)};
 
   Ray<f32x2> ray;
   ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = f32x2(0.0f);

@@ -74,7 +74,7 @@ template <> __device__ __forceinline__ float fma_<float>(float a, float b, float
 
 // Spin-dependent constants, computed once on the host.
 template <typename T> struct SpinConst {
-  T a, a2, two_a, two_a2;
+  T a, a2, two_a, two_a2, four_a2;
 };
 
 // Position-only part of the right-hand side (shared by the stopping test, the step rule and stage 1).
@@ -89,8 +89,8 @@ template <typename T> struct SpinConst {
 // never formed.
 template <typename T> struct Geometry {
   T r, rinv, Pinv, hf, f, l3, zeta;
-  T alpha, beta, lf;        // grad f = alpha n - beta e_z ;  lf = l . grad f
-  T tr, trP, rP, taP;       // 2r, 2r/P, r/P, 2a/P
+  T fc1, beta, lf;          // grad f = f c1 (f/2) n - beta e_z ;  lf = l . grad f = f c1 - beta l3
+  T trP, rP, taP;           // 2r/P, r/P, 2a/P
 };
 
 template <typename T>
@@ -117,17 +117,13 @@ __device__ __forceinline__ void ks_geometry(const SpinConst<T> &k, T x, T y, T z
   g.hf = hf;
   g.f = f;
   g.l3 = z * rinv;
-  T rinv2 = rinv * rinv;
-  g.zeta = z * (P * rinv2);
+  g.zeta = (P * rinv) * g.l3;                      // z P / r^2
   T c1 = fma_(T(3), rinv, -(f + f));
-  T c2 = k.two_a2 * z * (Dinv * rinv2);
-  T fc1 = f * c1;
-  g.alpha = fc1 * hf;
-  g.beta = c2 * f;
-  g.lf = fma_(-g.beta, g.l3, fc1);
-  g.tr = r + r;
-  g.trP = g.tr * Pinv;
+  g.fc1 = f * c1;
+  g.beta = (k.four_a2 * g.l3) * (Dinv * Dinv);     // f c2 = (2r/D) 2a^2 z/(D r^2) = 4 a^2 l3 / D^2
+  g.lf = fma_(-g.beta, g.l3, g.fc1);
   g.rP = r * Pinv;
+  g.trP = g.rP + g.rP;
   g.taP = k.two_a * Pinv;
 }
 
@@ -138,19 +134,18 @@ __device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T
   T xu = fma_(x, u1, y * u2);
   T yu = fma_(y, u1, -x * u2);
   T Lu = fma_(g.r, xu, k.a * yu);
-  T lu = g.Pinv * Lu;                              // l1 u1 + l2 u2
-  T zu = g.l3 * u3;
-  T U = fma_(g.l3, u3, fma_(g.Pinv, Lu, u0));      // l_alpha u^alpha
-  T Au = fma_(g.Pinv, fma_(-g.tr, lu, xu), -zu * g.rinv);
+  T w3 = u3 * g.rinv;
+  T U = fma_(g.l3, u3, fma_(g.Pinv, Lu, u0));      // l_alpha u^alpha ; l1 u1 + l2 u2 = Lu / P
+  T Au = fma_(g.Pinv, fma_(-g.trP, Lu, xu), -(g.l3 * w3));
   T unv = fma_(g.zeta, u3, xu);                    // n . u
   T ur = g.hf * unv;                               // u . grad r
   T s12 = fma_(u1, u1, u2 * u2);
-  T q = fma_(ur, Au, fma_(g.rP, s12, (u3 * u3) * g.rinv));
-  T uf = fma_(g.alpha, unv, -g.beta * u3);         // u . grad f
+  T q = fma_(ur, Au, fma_(g.rP, s12, u3 * w3));
+  T uf = fma_(g.fc1, ur, -g.beta * u3);            // u . grad f   (alpha n.u = f c1 u.grad r)
   T hU2 = T(0.5) * (U * U);
   T fU = g.f * U;
-  a0 = fma_(g.f * hU2, g.lf, fma_(U, uf, g.f * q));
-  T cn = fma_(fU * g.hf, Au, hU2 * g.alpha);
+  a0 = fma_(g.f, fma_(hU2, g.lf, q), U * uf);
+  T cn = g.hf * fma_(fU, Au, hU2 * g.fc1);         // f U (f/2) A.u + (U^2/2) alpha
   T cA = fU * ur;
   T cB = fU * g.taP;
   T e2 = g.Pinv * fma_(cA, g.trP, -a0);

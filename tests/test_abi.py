@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol(lib):
     for name in declared_functions():
         assert hasattr(lib, name), name
     assert b"sm_100a" in lib.gray2_version()
-    assert lib.gray2_flops_per_step(0) == 558 and lib.gray2_flops_per_step(1) == 558
+    assert lib.gray2_flops_per_step(0) == 530 and lib.gray2_flops_per_step(1) == 530
 
 
 def test_struct_layouts_match_the_header(lib):
