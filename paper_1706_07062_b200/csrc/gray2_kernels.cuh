@@ -166,8 +166,8 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
         U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
       }
       // NaN fails every compare; r_escape_fin = min(r_escape, largest finite) so that r = inf fails too
-      bool go = (g.r >= p.r_capture) && (g.r <= p.r_escape_fin) && fastmath<T>::finite(U) &&
-                fastmath<T>::finite(ray.t) && (nst < p.max_steps);
+      bool go = fastmath<T>::ge_pos(g.r, p.r_capture) && fastmath<T>::le_pos(g.r, p.r_escape_fin) &&
+                fastmath<T>::finite(U) && fastmath<T>::finite(ray.t) && (nst < p.max_steps);
       if (CLIP) go = go && (p.dir * (p.lambda_end - lam) > 0.0);
       if constexpr (FORM == 2) go = go && !cap;
       if (__any_sync(0xffffffffu, have && !go)) {

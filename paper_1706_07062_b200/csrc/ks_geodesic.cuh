@@ -51,7 +51,13 @@ template <> struct fastmath<double> {
     double t = fma(e, e, e);                   // y <- y (1 + e + e^2)
     return fma(y, t, y);
   }
-  static __device__ __forceinline__ bool finite(double x) { return fabs(x) <= 1.7976931348623157e308; }
+  // The stopping tests of the hot loop run on the integer pipe (the FP64 pipe is the one that is full):
+  // finite <=> exponent field not all ones; and for a >= 0 or NaN, b > 0 finite, the IEEE order of a and b
+  // is the order of their bit patterns -- a NaN compares above every finite b, so it fails the `le` test
+  // that always accompanies the `ge` test (a NaN with the sign bit set fails `ge`).
+  static __device__ __forceinline__ bool finite(double x) { return (__double2hiint(x) & 0x7ff00000) != 0x7ff00000; }
+  static __device__ __forceinline__ bool ge_pos(double a, double b) { return __double_as_longlong(a) >= __double_as_longlong(b); }
+  static __device__ __forceinline__ bool le_pos(double a, double b) { return __double_as_longlong(a) <= __double_as_longlong(b); }
 };
 
 template <> struct fastmath<float> {
@@ -66,6 +72,8 @@ template <> struct fastmath<float> {
     return y;
   }
   static __device__ __forceinline__ bool finite(float x) { return fabsf(x) <= 3.402823466e38f; }
+  static __device__ __forceinline__ bool ge_pos(float a, float b) { return a >= b; }
+  static __device__ __forceinline__ bool le_pos(float a, float b) { return a <= b; }
 };
 
 template <typename T> __device__ __forceinline__ T fma_(T a, T b, T c);
