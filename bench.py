@@ -39,10 +39,10 @@ INF = float("inf")
 FP_LANES = {"f64": 64, "f32": 128}
 
 # DRAM traffic of the dominant kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch, from the
-# `ncu --set full` captures summarised in profiles/r01_ncu_integrate_f{64,32}_v3.txt (cfg3, affine form) and
+# `ncu --set full` captures summarised in profiles/r01_ncu_integrate_f{64,32}_v4.txt (cfg3, affine form) and
 # profiles/r01_ncu_integrate_bl_f{64,32}.txt (cfg3, Boyer-Lindquist form).
 # Algorithmic state traffic is 2 x 80 B (FP64) or 2 x 48 B (FP32) per ray.
-NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83903744 + 31966464, ("cfg3", "f32", "affine"): 50362880 + 1761536,
+NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83935744 + 31088896, ("cfg3", "f32", "affine"): 50348544 + 1701632,
                   ("cfg3", "f64", "bl"): 84328448 + 31719936, ("cfg3", "f32", "bl"): 50350336 + 1810176}
 
 
