@@ -157,13 +157,15 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
     // ---- step all lanes until one of them has to stop ---------------------------------------------
     for (;;) {
       Geometry<T> g;
+      Vel<T> w;
       T U;
       if constexpr (FORM == 2) {
         g.r = ray.x;
         U = bl_probe(ray);
       } else {
         ks_geometry(k, ray.x, ray.y, ray.z, g);
-        U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+        w = ks_vel(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);     // reused by stage 1 of the step
+        U = w.U;
       }
       // NaN fails every compare; r_escape_fin = min(r_escape, largest finite) so that r = inf fails too
       bool go = fastmath<T>::ge_pos(g.r, p.r_capture) && fastmath<T>::le_pos(g.r, p.r_escape_fin) &&
@@ -203,8 +205,8 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
         if (rmin < p.r_capture) cap = true;
         else { ray = nxt; lam += hd; nst += 1; }
       } else {
-        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
-        else rk4_step(k, ray, g, h);
+        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, w, h);
+        else rk4_step(k, ray, g, w, h);
         lam += hd;
         nst += 1;
       }
@@ -312,13 +314,15 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
 
     for (;;) {
       Geometry<f32x2> g;
+      Vel<f32x2> w;
       f32x2 U;
       if constexpr (FORM == 2) {
         g.r = ray.x;
         U = bl_probe(ray);
       } else {
         ks_geometry(k, ray.x, ray.y, ray.z, g);
-        U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+        w = ks_vel(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+        U = w.U;
       }
       bool stopA = A.have && !slot_may_step<0, CLIP>(p, g, U, ray, A);
       bool stopB = B.have && !slot_may_step<1, CLIP>(p, g, U, ray, B);
@@ -342,8 +346,8 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
         if (rmin.v.y < p.r_capture) B.cap = true;
         else { copy_half<1>(ray, nxt); B.lam += hdB; B.nst += 1; }
       } else {
-        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, h);
-        else rk4_step(k, ray, g, h);
+        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, w, h);
+        else rk4_step(k, ray, g, w, h);
         A.lam += hdA; B.lam += hdB;
         A.nst += 1; B.nst += 1;
       }
@@ -394,7 +398,8 @@ __global__ void integrate_diag_kernel(StateView<T> s, uint64_t n, StepParams<T> 
   for (;;) {
     Geometry<T> g;
     ks_geometry(k, ray.x, ray.y, ray.z, g);
-    T U = ks_U(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+    const Vel<T> w = ks_vel(k, g, ray.x, ray.y, ray.u0, ray.u1, ray.u2, ray.u3);
+    const T U = w.U;
     if (!(fastmath<T>::finite(g.r) && fastmath<T>::finite(U) && fastmath<T>::finite(ray.t))) { st = GRAY2_INVALID; break; }
     {   // ---- sample k ----
       double u0 = (double)ray.u0, u1 = (double)ray.u1, u2 = (double)ray.u2, u3 = (double)ray.u3;
@@ -433,7 +438,7 @@ __global__ void integrate_diag_kernel(StateView<T> s, uint64_t n, StepParams<T> 
     T h = (MODE == 1) ? p.eta_or_h * g.r : p.eta_or_h;
     double hd = (double)h, rem = p.lambda_end - lam;
     if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
-    rk4_step(k, ray, g, h);
+    rk4_step(k, ray, g, w, h);
     lam += hd;
     nst += 1;
   }

@@ -135,15 +135,28 @@ __device__ __forceinline__ void ks_geometry(const SpinConst<T> &k, T x, T y, T z
   g.taP = k.two_a * Pinv;
 }
 
+// The first products of the velocity-dependent part.  U = l_alpha u^alpha also serves as the finiteness probe
+// of the stopping test, so the kernels evaluate this once at the top of a step and hand it to stage 1.
+template <typename T> struct Vel {
+  T xu, Lu, U;              // x u1 + y u2 ;  P (l1 u1 + l2 u2) ;  l_alpha u^alpha
+};
+
+template <typename T>
+__device__ __forceinline__ Vel<T> ks_vel(const SpinConst<T> &k, const Geometry<T> &g, T x, T y, T u0, T u1, T u2, T u3) {
+  Vel<T> w;
+  w.xu = fma_(x, u1, y * u2);
+  T yu = fma_(y, u1, -x * u2);
+  w.Lu = fma_(g.r, w.xu, k.a * yu);
+  w.U = fma_(g.l3, u3, fma_(g.Pinv, w.Lu, u0));
+  return w;
+}
+
 // Velocity-dependent part: xddot^mu from the geometry, the position and u (eq. 13-14).
 template <typename T>
-__device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T> &g, T x, T y,
-                                         T u0, T u1, T u2, T u3, T &a0, T &a1, T &a2, T &a3) {
-  T xu = fma_(x, u1, y * u2);
-  T yu = fma_(y, u1, -x * u2);
-  T Lu = fma_(g.r, xu, k.a * yu);
+__device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T> &g, const Vel<T> &w, T x, T y,
+                                         T u1, T u2, T u3, T &a0, T &a1, T &a2, T &a3) {
+  const T xu = w.xu, Lu = w.Lu, U = w.U;
   T w3 = u3 * g.rinv;
-  T U = fma_(g.l3, u3, fma_(g.Pinv, Lu, u0));      // l_alpha u^alpha ; l1 u1 + l2 u2 = Lu / P
   T Au = fma_(g.Pinv, fma_(-g.trP, Lu, xu), -(g.l3 * w3));
   T unv = fma_(g.zeta, u3, xu);                    // n . u
   T ur = g.hf * unv;                               // u . grad r
@@ -164,13 +177,10 @@ __device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T
   a3 = fma_(cn, g.zeta, fma_(g.l3, fma_(cA, g.rinv, -a0), -hU2 * g.beta));
 }
 
-// l_alpha u^alpha alone (finite-ness test of the velocity at the top of a step).
 template <typename T>
-__device__ __forceinline__ T ks_U(const SpinConst<T> &k, const Geometry<T> &g, T x, T y, T u0, T u1, T u2, T u3) {
-  T xu = fma_(x, u1, y * u2);
-  T yu = fma_(y, u1, -x * u2);
-  T Lu = fma_(g.r, xu, k.a * yu);
-  return fma_(g.l3, u3, fma_(g.Pinv, Lu, u0));
+__device__ __forceinline__ void ks_accel(const SpinConst<T> &k, const Geometry<T> &g, T x, T y,
+                                         T u0, T u1, T u2, T u3, T &a0, T &a1, T &a2, T &a3) {
+  ks_accel(k, g, ks_vel(k, g, x, y, u0, u1, u2, u3), x, y, u1, u2, u3, a0, a1, a2, a3);
 }
 
 // One geodesic's 8 variables.
@@ -181,7 +191,7 @@ template <typename T> struct Ray {
 // Classic RK4.  `g1` is the geometry at the current position (already needed by the
 // stopping test and the step rule), so stage 1 costs only the velocity-dependent part.
 template <typename T>
-__device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, T h) {
+__device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, const Vel<T> &w1, T h) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
   T b0, b1, b2, b3;                      // stage acceleration
   T v0, v1, v2, v3;                      // stage velocity
@@ -189,7 +199,7 @@ __device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const
   T St, Sx, Sy, Sz, S0, S1, S2, S3;      // k1 + 2 k2 + 2 k3 (+ k4)
   Geometry<T> g;
   // stage 1
-  ks_accel(k, g1, s.x, s.y, s.u0, s.u1, s.u2, s.u3, b0, b1, b2, b3);
+  ks_accel(k, g1, w1, s.x, s.y, s.u1, s.u2, s.u3, b0, b1, b2, b3);
   St = s.u0; Sx = s.u1; Sy = s.u2; Sz = s.u3;
   S0 = b0; S1 = b1; S2 = b2; S3 = b3;
   px = fma_(hh, s.u1, s.x); py = fma_(hh, s.u2, s.y); pz = fma_(hh, s.u3, s.z);
@@ -225,10 +235,10 @@ __device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const
 // v^mu = dx^mu/dt, v^0 = 1.  PAPER.md:146 eq. (18): the right-hand side is the affine one evaluated with
 // u = (1, v) and recombined,  dv^i/dt = xddot^i - xddot^0 v^i  -- "the same computational complexity".
 template <typename T>
-__device__ __forceinline__ void ks_accel_coordtime(const SpinConst<T> &k, const Geometry<T> &g, T x, T y,
+__device__ __forceinline__ void ks_accel_coordtime(const SpinConst<T> &k, const Geometry<T> &g, const Vel<T> &w, T x, T y,
                                                    T v1, T v2, T v3, T &d1, T &d2, T &d3) {
   T a0, a1, a2, a3;
-  ks_accel(k, g, x, y, T(1), v1, v2, v3, a0, a1, a2, a3);
+  ks_accel(k, g, w, x, y, v1, v2, v3, a0, a1, a2, a3);
   d1 = fma_(-a0, v1, a1);
   d2 = fma_(-a0, v2, a2);
   d3 = fma_(-a0, v3, a3);
@@ -237,29 +247,29 @@ __device__ __forceinline__ void ks_accel_coordtime(const SpinConst<T> &k, const 
 // Classic RK4 in t of the six variables (x, v); uses Ray<T> with u0 unused (v^0 = 1) and t advanced by
 // the caller (t += h exactly).
 template <typename T>
-__device__ __forceinline__ void rk4_step_coordtime(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, T h) {
+__device__ __forceinline__ void rk4_step_coordtime(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, const Vel<T> &w1, T h) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
   T b1, b2, b3, v1, v2, v3, px, py, pz;
   T Sx, Sy, Sz, S1, S2, S3;
   Geometry<T> g;
-  ks_accel_coordtime(k, g1, s.x, s.y, s.u1, s.u2, s.u3, b1, b2, b3);
+  ks_accel_coordtime(k, g1, w1, s.x, s.y, s.u1, s.u2, s.u3, b1, b2, b3);
   Sx = s.u1; Sy = s.u2; Sz = s.u3; S1 = b1; S2 = b2; S3 = b3;
   px = fma_(hh, s.u1, s.x); py = fma_(hh, s.u2, s.y); pz = fma_(hh, s.u3, s.z);
   v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
   ks_geometry(k, px, py, pz, g);
-  ks_accel_coordtime(k, g, px, py, v1, v2, v3, b1, b2, b3);
+  ks_accel_coordtime(k, g, ks_vel(k, g, px, py, T(1), v1, v2, v3), px, py, v1, v2, v3, b1, b2, b3);
   Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
   S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
   px = fma_(hh, v1, s.x); py = fma_(hh, v2, s.y); pz = fma_(hh, v3, s.z);
   v1 = fma_(hh, b1, s.u1); v2 = fma_(hh, b2, s.u2); v3 = fma_(hh, b3, s.u3);
   ks_geometry(k, px, py, pz, g);
-  ks_accel_coordtime(k, g, px, py, v1, v2, v3, b1, b2, b3);
+  ks_accel_coordtime(k, g, ks_vel(k, g, px, py, T(1), v1, v2, v3), px, py, v1, v2, v3, b1, b2, b3);
   Sx = fma_(T(2), v1, Sx); Sy = fma_(T(2), v2, Sy); Sz = fma_(T(2), v3, Sz);
   S1 = fma_(T(2), b1, S1); S2 = fma_(T(2), b2, S2); S3 = fma_(T(2), b3, S3);
   px = fma_(h, v1, s.x); py = fma_(h, v2, s.y); pz = fma_(h, v3, s.z);
   v1 = fma_(h, b1, s.u1); v2 = fma_(h, b2, s.u2); v3 = fma_(h, b3, s.u3);
   ks_geometry(k, px, py, pz, g);
-  ks_accel_coordtime(k, g, px, py, v1, v2, v3, b1, b2, b3);
+  ks_accel_coordtime(k, g, ks_vel(k, g, px, py, T(1), v1, v2, v3), px, py, v1, v2, v3, b1, b2, b3);
   s.x = fma_(h6, Sx + v1, s.x); s.y = fma_(h6, Sy + v2, s.y); s.z = fma_(h6, Sz + v3, s.z);
   s.u1 = fma_(h6, S1 + b1, s.u1); s.u2 = fma_(h6, S2 + b2, s.u2); s.u3 = fma_(h6, S3 + b3, s.u3);
 }
