@@ -43,7 +43,7 @@ FP_LANES = {"f64": 64, "f32": 128}
 # profiles/r01_ncu_integrate_bl_f{64,32}.txt (cfg3, Boyer-Lindquist form).
 # Algorithmic state traffic is 2 x 80 B (FP64) or 2 x 48 B (FP32) per ray.
 NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83935744 + 31088896, ("cfg3", "f32", "affine"): 50348544 + 1701632,
-                  ("cfg3", "f64", "bl"): 84328448 + 31719936, ("cfg3", "f32", "bl"): 50350336 + 1810176}
+                  ("cfg3", "f64", "bl"): 83937280 + 34206208, ("cfg3", "f32", "bl"): 50350080 + 1716480}
 
 
 def nominal_peak_tflops(dtype: str, n_sms: int, sm_max_mhz: float) -> float:

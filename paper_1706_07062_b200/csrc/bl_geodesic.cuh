@@ -98,25 +98,28 @@ __device__ __forceinline__ void bl_accel(const SpinConst<T> &k, T r, T th, T u0,
   const T iS = fastmath<T>::rcp(Sig), iD = fastmath<T>::rcp(Dl), iP = fastmath<T>::rcp(P), is2 = fastmath<T>::rcp(s2);
   const T A = tr * iS;
   const T B = (k.two_a2 * sc) * iS;
-  const T om = fma_(-(k.a * s2), u3, u0);
+  const T as2 = k.a * s2;
+  const T om = fma_(-as2, u3, u0);
   const T W = A * om;
   const T Ar = fma_(-A, A, iS + iS);
   const T AB = A * B;
-  const T Ad = fma_(Ar, u1, AB * u2);
-  const T ru1 = r * u1;
-  const T X1 = fma_((k.a * sc) * u2, W, -((s2 * ru1) * u3));
-  const T Wd = fma_(P * Ad, om, -((k.two_a * A) * X1)) * iD;
+  const T Bu2 = B * u2;
+  const T Ad = fma_(Ar, u1, A * Bu2);
+  const T tru1 = tr * u1;
+  const T tru1u3 = tru1 * u3;
+  // 2aA (a sin cos th' W - sin^2 r r' ph') = (B th') (2r W) - (a sin^2 A) (2r r' ph')   since A Sigma = 2r
+  const T Wd = fma_(as2 * A, tru1u3, fma_(-Bu2, tr * W, (P * Ad) * om)) * iD;
   a0 = Wd;
   const T cot2 = (sc + sc) * is2;
   const T Y = fma_(k.a, W, -(P * u3));
-  a3 = iP * fma_(k.a, Wd, fma_(cot2 * u2, Y, -((tr * u1) * u3)));
+  a3 = iP * fma_(k.a, Wd, fma_(cot2 * u2, Y, -tru1u3));
   const T om2h = (T(0.5) * om) * om;
   const T u1s = u1 * u1, u2s = u2 * u2;
   const T Kk = fma_(s2 * u3, u3, u2s);
   const T M = fma_(r, Kk, Ar * om2h);
   const T G = fma_(r, iS, -((r + T(-1)) * iD));
-  a1 = fma_(Dl * iS, M, fma_(-G, u1s, (B * u2) * u1));
-  const T N = fma_(sc * u3, fma_(P, u3, -(k.two_a * W)), fma_(AB, om2h, -(tr * u1) * u2));
+  a1 = fma_(Dl * iS, M, fma_(-G, u1s, Bu2 * u1));
+  const T N = fma_(sc * u3, fma_(P, u3, -(k.two_a * W)), fma_(AB, om2h, -tru1 * u2));
   a2 = fma_(iS, N, -((T(0.5) * B) * fma_(u1s, iD, -u2s)));
 }
 

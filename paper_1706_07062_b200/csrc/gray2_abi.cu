@@ -485,9 +485,9 @@ int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 534; }
 /* Boyer-Lindquist form, source-level count of bl_geodesic.cuh (same conventions):
  *   sin^2 and sin cos of theta: reduction 8, series 17 + 16, products 2 -> 43 (double: 8 / 8 terms, period pi/2),
  *                               reduction 8, series 13 + 12, products 2 -> 35 (float: 6 / 6 terms, period pi)
- *   rest of the right-hand side 87 (4 of them reciprocals)  ->  130 / 122 per right-hand side
- *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 622 / 590 per step. */
-int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 590 : 622; }
+ *   rest of the right-hand side 81 (4 of them reciprocals)  ->  124 / 116 per right-hand side
+ *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 598 / 566 per step. */
+int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 566 : 598; }
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
