@@ -141,7 +141,8 @@ int gray2_integrate(gray2_state *s, uint64_t n, double lambda_end, const gray2_s
  * a^2 = 1); velocities are mapped with the Jacobian.  theta in [0, pi], phi in the principal range on output.
  * Evaluated in double whatever the precision of the state.  dst: caller-owned arrays of the same precision
  * as src (dst->q.., lambda, status, nsteps, n, prec filled by the caller); on return dst->coords = to_coords
- * and a_eff, kind, reversed, lambda, status, nsteps are copied.  src and dst must not alias.  On the axis
+ * and a_eff, kind, reversed, lambda, status, nsteps are copied.  dst may be src itself (each geodesic is read
+ * completely before it is written); partial overlap is not allowed.  On the axis
  * the BL velocity is not finite (data, not an error).  GRAY2_EINVAL if src is already in to_coords. */
 int gray2_convert(const gray2_state *src, gray2_state *dst, uint64_t n, int32_t to_coords, void *cuda_stream);
 

@@ -418,23 +418,32 @@ int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, do
 int gray2_convert(const gray2_state *src, gray2_state *dst, uint64_t n, int32_t to_coords, void *cuda_stream) {
   int rc = check_state(src, "gray2_convert");
   if (rc) return rc;
-  if (dst) dst->coords = to_coords;
-  rc = check_state(dst, "gray2_convert");
-  if (rc) return rc;
+  if (to_coords != GRAY2_KS && to_coords != GRAY2_BL) return fail(GRAY2_EINVAL, "gray2_convert: unknown coordinates %d", to_coords);
   if (src->coords == to_coords) return fail(GRAY2_EINVAL, "gray2_convert: the state is already in those coordinates");
+  if (!dst) return fail(GRAY2_EINVAL, "gray2_convert: dst is NULL");
+  {
+    gray2_state probe = *dst;              // dst->coords is an output: validate the rest (dst may be src itself)
+    probe.coords = to_coords;
+    rc = check_state(&probe, "gray2_convert");
+    if (rc) return rc;
+  }
   if (src->prec != dst->prec) return fail(GRAY2_EINVAL, "gray2_convert: src and dst differ in precision");
   if (n == 0) return fail(GRAY2_EINVAL, "gray2_convert: n == 0");
   if (n > src->n || n > dst->n) return fail(GRAY2_ESTATE, "gray2_convert: n exceeds the size of src or dst");
   if (!(fabs(src->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_convert: |a_eff| must be <= 1");
-  dst->a_eff = src->a_eff; dst->kind = src->kind; dst->reversed = src->reversed;
+  const double a = src->a_eff;
+  const int32_t prec = src->prec;
+  const auto vs64 = view_of<double>(src), vd64 = view_of<double>(dst);
+  const auto vs32 = view_of<float>(src), vd32 = view_of<float>(dst);
+  dst->a_eff = src->a_eff; dst->kind = src->kind; dst->reversed = src->reversed; dst->coords = to_coords;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   unsigned grid = (unsigned)((n + 255) / 256);
   if (to_coords == GRAY2_BL) {
-    if (src->prec == GRAY2_F64) gray2::ks_to_bl_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(src), view_of<double>(dst), n, src->a_eff);
-    else gray2::ks_to_bl_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(src), view_of<float>(dst), n, src->a_eff);
+    if (prec == GRAY2_F64) gray2::ks_to_bl_kernel<double><<<grid, 256, 0, st>>>(vs64, vd64, n, a);
+    else gray2::ks_to_bl_kernel<float><<<grid, 256, 0, st>>>(vs32, vd32, n, a);
   } else {
-    if (src->prec == GRAY2_F64) gray2::bl_to_ks_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(src), view_of<double>(dst), n, src->a_eff);
-    else gray2::bl_to_ks_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(src), view_of<float>(dst), n, src->a_eff);
+    if (prec == GRAY2_F64) gray2::bl_to_ks_kernel<double><<<grid, 256, 0, st>>>(vs64, vd64, n, a);
+    else gray2::bl_to_ks_kernel<float><<<grid, 256, 0, st>>>(vs32, vd32, n, a);
   }
   CUDA_TRY(cudaGetLastError());
   return GRAY2_OK;

@@ -90,6 +90,16 @@ def test_convert_near_the_hole_timelike_and_fp32():
     assert state_rel_error_bl(gb32.q.double().cpu().numpy(), ob.q).max() < 2e-6
 
 
+def test_convert_in_place():
+    cfg = inputs.CFG3_NULL.scaled(50, 40)
+    g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    ref = gray2.convert(g, gray2.BL)
+    same = gray2.convert(g, gray2.BL, out=g)            # dst is src
+    assert same is g and g.coords == gray2.BL and torch.equal(g.q, ref.q)
+    back = gray2.convert(g, gray2.KS, out=g)
+    assert back.coords == gray2.KS and torch.equal(back.q, gray2.convert(ref, gray2.KS).q)
+
+
 def test_convert_and_coords_argument_checks():
     g = gray2.init_null(0.5, 1000.0, 1.0, 5.0, 5.0, 8, 8)
     with pytest.raises(gray2.Gray2Error) as e:
