@@ -92,3 +92,67 @@ def test_product_path_does_not_import_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text, f
                 assert "gray2_oracle" not in text, f
+
+
+def test_new_entries_reject_bad_arguments_without_gpu_work(lib):
+    from paper_1706_07062_b200 import gray2
+    EINVAL, ESTATE = 1, 2
+    null = C.c_void_p(0)
+    assert gray2._CState.coords.offset == 116 and gray2._CState.reversed.offset == 112
+    s = gray2._CState()
+    s.n, s.prec = 16, 0
+    for m in range(8):
+        s.q[m] = 0x1000
+    s.lam = s.status = s.nsteps = 0x1000
+    d = gray2._CState()
+    C.memmove(C.byref(d), C.byref(s), C.sizeof(s))
+    assert lib.gray2_convert(C.byref(s), C.byref(d), 16, 0, null) == EINVAL          # already Kerr-Schild
+    assert lib.gray2_convert(C.byref(s), C.byref(d), 16, 5, null) == EINVAL          # unknown coordinates
+    assert lib.gray2_convert(C.byref(s), null, 16, 1, null) == EINVAL
+    assert lib.gray2_convert(C.byref(s), C.byref(d), 17, 1, null) == ESTATE
+    d.prec = 1
+    assert lib.gray2_convert(C.byref(s), C.byref(d), 16, 1, null) == EINVAL          # precision mismatch
+    assert d.coords == 0                                                              # dst untouched on error
+    s.coords = 9
+    sc = gray2.step_control(mode=1, eta=0.01)
+    assert lib.gray2_integrate(C.byref(s), 16, 1.0, C.byref(sc), 0, null, null) == EINVAL
+    s.coords = 1                                                                       # Boyer-Lindquist state
+    assert lib.gray2_integrate_coordtime(C.byref(s), 16, 1.0, C.byref(sc), 0, null, null) == EINVAL
+    s.coords = 0
+    lib.gray2_init_null_shard.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                          C.c_int32, C.c_int32, C.c_uint64, C.c_int32, C.c_int32, C.c_void_p]
+    args = (0.5, 100.0, 1.0, 10.0, 10.0, 8, 4)
+    assert lib.gray2_init_null_shard(C.byref(s), *args, 0, 0, 2, null) == EINVAL      # tile_rays == 0
+    assert lib.gray2_init_null_shard(C.byref(s), *args, 8, 2, 2, null) == EINVAL      # rank >= world
+    s.n = 15
+    assert lib.gray2_init_null_shard(C.byref(s), *args, 8, 0, 2, null) == EINVAL      # shard has 16 rays, state 15
+    assert lib.gray2_rhs_bl(0, 0.5, 0, null, null, null, null) == EINVAL
+    assert lib.gray2_flops_per_step_bl(0) == 598 and lib.gray2_flops_per_step_bl(1) == 566
+    assert lib.gray2_flops_per_step_coordtime(0) == 534
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    import json
+    import subprocess
+    import sys
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0", "--oracle-side", "16"], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-500:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["vs_baseline"] is None and line["higher_is_better"] is True
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "scaling", "dtype", "data", "config"):
+        assert key in line, key
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] == line["value"]
+    assert line["e2e"] == {"value": line["value"], "unit": line["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert line["value"] > 1e4 and line["config"]["rays"] == 256
+
+
+def test_bench_gpu_arm_fails_loudly_without_a_gpu():
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1"], capture_output=True,
+                         text=True, timeout=300)
+    assert out.returncode != 0 and "no CPU fallback" in (out.stderr + out.stdout)
