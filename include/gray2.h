@@ -21,8 +21,9 @@
  *
  * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
  * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
- * library allocates no device memory of its own except a 4 KiB work-queue scratch and the staging buffer
- * of gray2_init_timelike (n x 64 bytes, grown on demand, reused, released at process exit).  `host_xu8` is a HOST pointer.
+ * library allocates no device memory of its own except a 4 KiB work-queue scratch and the staging buffers
+ * of gray2_init_timelike (n x 64 bytes each, one per calling stream up to eight, grown on demand, reused,
+ * released at process exit).  `host_xu8` is a HOST pointer.
  * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
  *
  * Asynchrony.  Every call enqueues on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
@@ -113,7 +114,9 @@ uint64_t gray2_shard_count(uint64_t n, uint64_t tile_rays, int32_t rank, int32_t
  * Copies them into the first n slots of the SoA state (converted to float for F32); with
  * renormalise_ut != 0 replaces u^t by the future-directed root of g u u = -1 (R7).  Sets s->a_eff = a,
  * s->kind = GRAY2_TIMELIKE, s->reversed = 0, lambda = 0, status = ACTIVE, nsteps = 0.  The host array
- * may be reused as soon as the call returns (the call synchronises its staging copy). */
+ * may be reused as soon as the call returns: the call waits for its own host-to-device copy (made on an
+ * internal stream, so that it does not queue behind earlier work on cuda_stream) and for nothing else; the
+ * state is filled in stream order on cuda_stream like the output of every other call. */
 int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n,
                         int32_t renormalise_ut, void *cuda_stream);
 

@@ -304,30 +304,55 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
   if (n > s->n) return fail(GRAY2_ESTATE, "gray2_init_timelike: n (%llu) exceeds s->n (%llu)", (unsigned long long)n, (unsigned long long)s->n);
   if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_timelike: |a| must be <= 1 (got %g)", a);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  // Staging buffer for the AoS input: owned by the library, grown on demand and reused (a fresh
-  // stream-ordered allocation per call costs up to 100 ms when the pool has to grow again).  The lock is
-  // held until the stream has been synchronised, so concurrent callers cannot overwrite each other's input.
+  // Staging buffers for the AoS input: owned by the library, grown on demand and reused (a fresh
+  // stream-ordered allocation per call costs up to 100 ms when the pool has to grow again).  A small pool,
+  // one slot per calling stream (round robin beyond kStages streams).  The host-to-device copy runs on an
+  // internal stream, so that it does not queue behind the caller's earlier work on `st` (a caller that
+  // pipelines chunks over a few streams gets its inputs prefetched while earlier chunks integrate); the
+  // caller's stream waits for the copy, the next copy into a slot waits for the kernel that consumed it, and
+  // the host waits only for its own copy, after which host_xu8 may be reused.
+  constexpr int kStages = 8;
+  struct Stage { cudaStream_t key; bool made; double *buf; size_t bytes; cudaEvent_t copied, consumed; };
   static std::mutex stage_lock;
-  static double *stage = nullptr;
-  static size_t stage_bytes = 0;
-  std::lock_guard<std::mutex> guard(stage_lock);
-  size_t bytes = (size_t)n * 8 * sizeof(double);
-  if (bytes > stage_bytes) {
-    if (stage) { cudaFree(stage); stage = nullptr; stage_bytes = 0; }
-    CUDA_TRY(cudaMalloc(&stage, bytes));
-    stage_bytes = bytes;
-  }
-  cudaError_t e = cudaMemcpyAsync(stage, host_xu8, bytes, cudaMemcpyHostToDevice, st);
-  if (e == cudaSuccess) {
+  static Stage stages[kStages] = {};
+  static cudaStream_t copy_stream = nullptr;
+  static unsigned next_slot = 0;
+  const size_t bytes = (size_t)n * 8 * sizeof(double);
+  cudaEvent_t copied;
+  {
+    std::lock_guard<std::mutex> guard(stage_lock);
+    if (!copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+    Stage *sl = nullptr;
+    for (int i = 0; i < kStages && !sl; ++i)
+      if (stages[i].made && stages[i].key == st) sl = &stages[i];
+    if (!sl) {
+      sl = &stages[next_slot++ % kStages];
+      if (!sl->made) {
+        CUDA_TRY(cudaEventCreateWithFlags(&sl->copied, cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&sl->consumed, cudaEventDisableTiming));
+        sl->made = true;
+      }
+      sl->key = st;
+    }
+    if (bytes > sl->bytes) {
+      if (sl->buf) { CUDA_TRY(cudaEventSynchronize(sl->consumed)); cudaFree(sl->buf); sl->buf = nullptr; sl->bytes = 0; }
+      CUDA_TRY(cudaMalloc(&sl->buf, bytes));
+      sl->bytes = bytes;
+    }
+    CUDA_TRY(cudaStreamWaitEvent(copy_stream, sl->consumed, 0));      // the kernel that last read this slot
+    CUDA_TRY(cudaMemcpyAsync(sl->buf, host_xu8, bytes, cudaMemcpyHostToDevice, copy_stream));
+    CUDA_TRY(cudaEventRecord(sl->copied, copy_stream));
+    CUDA_TRY(cudaStreamWaitEvent(st, sl->copied, 0));
     unsigned grid = (unsigned)((n + 255) / 256);
     if (s->prec == GRAY2_F64)
-      gray2::init_explicit_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), stage, n, a, renorm);
+      gray2::init_explicit_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), sl->buf, n, a, renorm);
     else
-      gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), stage, n, a, renorm);
-    e = cudaGetLastError();
+      gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), sl->buf, n, a, renorm);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaEventRecord(sl->consumed, st));
+    copied = sl->copied;
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the staging buffer and host_xu8 may be reused on return
-  if (e != cudaSuccess) return fail(GRAY2_ECUDA, "gray2_init_timelike: %s", cudaGetErrorString(e));
+  CUDA_TRY(cudaEventSynchronize(copied));   // host_xu8 may be reused on return
   s->a_eff = a; s->kind = GRAY2_TIMELIKE; s->reversed = 0; s->coords = GRAY2_KS;
   return GRAY2_OK;
 }
