@@ -273,13 +273,14 @@ def run_gpu(args):
     host_in.copy_(src.q.t())          # outside the timed region: the user's 8-vectors, resident in host memory
     a_eff = src.a_eff
     del src
-    # The batch is cut into chunks that alternate between two streams, so that the H2D copy of one chunk
+    # The batch is cut into chunks that alternate between a few streams, so that the H2D copy of one chunk
     # and the D2H copy of another overlap the integration of a third (every call below is the public API).
     # Each chunk has its own contiguous device state and pinned host result buffers, so every copy is a
     # plain asynchronous memcpy.
     n_chunks = max(1, args.e2e_chunks)
     bounds = [(n_local * c // n_chunks, n_local * (c + 1) // n_chunks) for c in range(n_chunks)]
-    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    n_streams = max(1, args.e2e_streams)
+    streams = [torch.cuda.Stream() for _ in range(n_streams)]
     host_in_np = host_in.numpy()
     parts, parts_ks, host_out, chunk_stats = [], [], [], []
     for lo, hi in bounds:
@@ -299,7 +300,7 @@ def run_gpu(args):
     def e2e_step():
         for c, (lo, hi) in enumerate(bounds):
             part, ho = parts[c], host_out[c]
-            with torch.cuda.stream(streams[c % 2]):
+            with torch.cuda.stream(streams[c % n_streams]):
                 if bl:
                     ks = parts_ks[c]
                     gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=ks)
@@ -362,7 +363,7 @@ def run_gpu(args):
             "clocks": clocks,
             "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "gray2_init_timelike(host 8-vectors) -> %sgray2_integrate -> gray2_invariants -> D2H of state, invariants, stats" % ("gray2_convert -> " if bl else ""),
-                    "chunks": n_chunks, "streams": 2},
+                    "chunks": n_chunks, "streams": n_streams},
             "gpu_launches": (5 if bl else 4) * args.steps,
             "roofline": {"bound": "alu", "kernel": ("integrate_kernel<double%s>" if prec == gray2.F64 else "integrate_kernel_f32x2<%s>") % (
                              ", coordinate time" if coord else ", Boyer-Lindquist" if bl else ("" if prec == gray2.F64 else "affine")),
@@ -407,7 +408,8 @@ def main():
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--blocks", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-chunks", type=int, default=8, help="end-to-end leg: chunks pipelined over two streams")
+    ap.add_argument("--e2e-chunks", type=int, default=8, help="end-to-end leg: chunks pipelined over the streams")
+    ap.add_argument("--e2e-streams", type=int, default=2, help="end-to-end leg: number of streams the chunks alternate between")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
