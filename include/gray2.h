@@ -21,10 +21,17 @@
  *
  * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
  * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
- * library allocates no device memory of its own except a 4 KiB work-queue scratch and the staging buffers
+ * library allocates no device memory of its own except a 4 KiB work-queue scratch per device (64 slots
+ * handed out round-robin; a call that gets a slot whose previous user is still running waits for it on
+ * the device, so any number of integrations may be in flight) and the staging buffers
  * of gray2_init_timelike (n x 64 bytes each, one per calling stream up to eight, grown on demand, reused,
  * released at process exit).  `host_xu8` is a HOST pointer.
  * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
+ *
+ * Devices.  Work runs on the CUDA device that is current in the calling thread; all pointers and the
+ * stream must belong to it.  The integrators may be used on several devices of one process (their scratch
+ * is per device); gray2_init_timelike keeps its staging buffers on the device of its first call, so a
+ * process that feeds explicit 8-vectors to several GPUs needs one process per GPU (the model of bench.py).
  *
  * Asynchrony.  Every call enqueues on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
  * stream) and returns; results are valid after the caller synchronises that stream.

@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgray2.so")
 SOURCES = [os.path.join(CSRC, "gray2_abi.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "gray2_kernels.cuh"), os.path.join(CSRC, "ks_geodesic.cuh"),
-                  os.path.join(os.path.dirname(HERE), "include", "gray2.h")]
+DEPS = SOURCES + [os.path.join(CSRC, h) for h in sorted(os.listdir(CSRC)) if h.endswith(".cuh")] + [
+    os.path.join(os.path.dirname(HERE), "include", "gray2.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--fmad=false",

@@ -7,7 +7,6 @@
 #include <stdio.h>
 #include <string.h>
 
-#include <atomic>
 #include <mutex>
 
 #include "../../include/gray2.h"
@@ -31,28 +30,53 @@ int fail(int code, const char *fmt, ...) {
     if (e_ != cudaSuccess) return fail(GRAY2_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
   } while (0)
 
-// ---- work-queue scratch: 64 counters, one 64-byte line each, handed out round-robin ---------------
+// ---- work-queue scratch: per device, 64 slots of one 64-byte line each, handed out round-robin ---------
+// Slot i holds the queue counter at word 8 i and the step counter at word 8 i + 1.  A slot is handed out
+// again only after 63 later calls; should the work that last used it still be running then (more than 64
+// integrations in flight on different streams), the new user's stream waits for it: every slot carries an
+// event recorded behind its last user.
 constexpr int kQueueSlots = 64;
-unsigned long long *g_queue = nullptr;   // device, kQueueSlots * 8 words (slot i at word 8 i; word 8 i + 1 = steps)
-std::atomic<unsigned> g_queue_next{0};
-std::atomic<int> g_queue_ready{0};
-int g_num_sms = 0;
+constexpr int kMaxDevices = 64;
+struct Scratch {
+  unsigned long long *queue = nullptr;       // device, kQueueSlots * 8 words
+  cudaEvent_t done[kQueueSlots] = {};        // recorded behind the last work that used the slot
+  unsigned next = 0;
+  int num_sms = 0;
+  bool ready = false;
+};
+Scratch g_scratch[kMaxDevices];
+std::mutex g_scratch_lock;
 
-int ensure_scratch() {
-  if (g_queue_ready.load(std::memory_order_acquire)) return GRAY2_OK;
-  static std::atomic_flag busy = ATOMIC_FLAG_INIT;
-  while (busy.test_and_set(std::memory_order_acquire)) {}
-  int rc = GRAY2_OK;
-  if (!g_queue_ready.load(std::memory_order_acquire)) {
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaMalloc(&g_queue, kQueueSlots * 8 * sizeof(unsigned long long));
-    if (e != cudaSuccess) rc = fail(GRAY2_ECUDA, "scratch allocation: %s", cudaGetErrorString(e));
-    else g_queue_ready.store(1, std::memory_order_release);
+struct QueueSlot {
+  unsigned long long *queue, *steps;
+  cudaEvent_t done;
+  int num_sms;
+};
+
+// Takes the next slot of the current device and makes `st` wait for the slot's previous user.
+int acquire_slot(cudaStream_t st, QueueSlot *out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(GRAY2_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kMaxDevices) return fail(GRAY2_ECUDA, "device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> guard(g_scratch_lock);
+  Scratch &sc = g_scratch[dev];
+  if (!sc.ready) {
+    e = cudaDeviceGetAttribute(&sc.num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess && !sc.queue) e = cudaMalloc(&sc.queue, kQueueSlots * 8 * sizeof(unsigned long long));
+    for (int i = 0; i < kQueueSlots && e == cudaSuccess; ++i)
+      if (!sc.done[i]) e = cudaEventCreateWithFlags(&sc.done[i], cudaEventDisableTiming);
+    if (e != cudaSuccess) return fail(GRAY2_ECUDA, "scratch allocation: %s", cudaGetErrorString(e));
+    sc.ready = true;
   }
-  busy.clear(std::memory_order_release);
-  return rc;
+  const unsigned slot = sc.next++ % kQueueSlots;
+  out->queue = sc.queue + 8 * slot;
+  out->steps = out->queue + 1;
+  out->done = sc.done[slot];
+  out->num_sms = sc.num_sms;
+  e = cudaStreamWaitEvent(st, out->done, 0);   // a never-recorded event is complete: no wait
+  if (e != cudaSuccess) return fail(GRAY2_ECUDA, "cudaStreamWaitEvent: %s", cudaGetErrorString(e));
+  return GRAY2_OK;
 }
 
 // ---- launch configuration of the integrator (gray2_set_launch) ------------------------------------
@@ -84,9 +108,9 @@ namespace {
 
 template <typename T, int THREADS, int MIN_BLOCKS, int FORM>
 cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::StepParams<T> &p,
-                             unsigned long long *queue, unsigned long long *steps, cudaStream_t st) {
+                             unsigned long long *queue, unsigned long long *steps, int num_sms, cudaStream_t st) {
   uint64_t want = (n + THREADS - 1) / THREADS;
-  uint64_t cap = (uint64_t)g_num_sms * MIN_BLOCKS;
+  uint64_t cap = (uint64_t)num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<T>(s);
   if (p.mode == 1) {
@@ -102,9 +126,9 @@ cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::Step
 // FP32 with two geodesics per thread (packed FP32x2 arithmetic)
 template <int THREADS, int MIN_BLOCKS, int FORM>
 cudaError_t launch_integrate_x2(const gray2_state *s, uint64_t n, const gray2::StepParams<float> &p,
-                                unsigned long long *queue, unsigned long long *steps, cudaStream_t st) {
+                                unsigned long long *queue, unsigned long long *steps, int num_sms, cudaStream_t st) {
   uint64_t want = (n + 2 * THREADS - 1) / (2 * THREADS);
-  uint64_t cap = (uint64_t)g_num_sms * MIN_BLOCKS;
+  uint64_t cap = (uint64_t)num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<float>(s);
   if (p.mode == 1) {
@@ -130,30 +154,30 @@ constexpr LaunchChoice kF32Variants[kNumVariants] = {{256, 2}, {128, 3}, {128, 4
 template <typename T>
 cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_state *s, uint64_t n,
                                const gray2::StepParams<T> &p, unsigned long long *q, unsigned long long *steps,
-                               cudaStream_t st, bool *found) {
+                               int sms, cudaStream_t st, bool *found) {
   *found = true;
   if constexpr (sizeof(T) == 8) {
-    if (form == 1) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, st);
+    if (form == 1) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, sms, st);
     if (form == 2) {
-      if (threads == 128 && blocks == 4) return launch_integrate<T, 128, 4, 2>(s, n, p, q, steps, st);
-      if (threads == 64 && blocks == 6) return launch_integrate<T, 64, 6, 2>(s, n, p, q, steps, st);
-      return launch_integrate<T, 128, 3, 2>(s, n, p, q, steps, st);
+      if (threads == 128 && blocks == 4) return launch_integrate<T, 128, 4, 2>(s, n, p, q, steps, sms, st);
+      if (threads == 64 && blocks == 6) return launch_integrate<T, 64, 6, 2>(s, n, p, q, steps, sms, st);
+      return launch_integrate<T, 128, 3, 2>(s, n, p, q, steps, sms, st);
     }
 #define GRAY2_VARIANT(TH, BL) \
-  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
+  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, sms, st);
     GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(128, 2)
 #undef GRAY2_VARIANT
   } else {
-    if (form == 1) return launch_integrate_x2<256, 2, 1>(s, n, p, q, steps, st);
+    if (form == 1) return launch_integrate_x2<256, 2, 1>(s, n, p, q, steps, sms, st);
     if (form == 2) {
-      if (threads == 128 && blocks == 4) return launch_integrate_x2<128, 4, 2>(s, n, p, q, steps, st);
-      if (threads == 128 && blocks == 3) return launch_integrate_x2<128, 3, 2>(s, n, p, q, steps, st);
-      return launch_integrate_x2<256, 2, 2>(s, n, p, q, steps, st);
+      if (threads == 128 && blocks == 4) return launch_integrate_x2<128, 4, 2>(s, n, p, q, steps, sms, st);
+      if (threads == 128 && blocks == 3) return launch_integrate_x2<128, 3, 2>(s, n, p, q, steps, sms, st);
+      return launch_integrate_x2<256, 2, 2>(s, n, p, q, steps, sms, st);
     }
 #define GRAY2_VARIANT_X2(TH, BL) \
-  if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, st);
+  if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, sms, st);
 #define GRAY2_VARIANT(TH, BL) \
-  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, st);
+  if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, sms, st);
     GRAY2_VARIANT_X2(128, 4) GRAY2_VARIANT_X2(128, 3) GRAY2_VARIANT_X2(256, 2)
     GRAY2_VARIANT(128, 8) GRAY2_VARIANT(128, 6)
 #undef GRAY2_VARIANT
@@ -182,8 +206,10 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, cons
   p.max_steps = sc->max_steps;
   p.clip = !(isinf(lambda_end) && (double)sc->dir * lambda_end > 0.0);
 
-  unsigned slot = g_queue_next.fetch_add(1) % kQueueSlots;
-  unsigned long long *queue = g_queue + 8 * slot, *steps = queue + 1;
+  QueueSlot qs;
+  int rc = acquire_slot(st, &qs);
+  if (rc) return rc;
+  unsigned long long *queue = qs.queue, *steps = qs.steps;
   CUDA_TRY(cudaMemsetAsync(queue, 0, 2 * sizeof(unsigned long long), st));
 
   const int pi = sizeof(T) == 8 ? 0 : 1;
@@ -191,7 +217,7 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, cons
   int threads = g_threads[pi] ? g_threads[pi] : def.threads;
   int blocks = g_blocks_per_sm[pi] ? g_blocks_per_sm[pi] : def.blocks;
   bool found = false;
-  cudaError_t e = dispatch_integrate<T>(form, threads, blocks, s, n, p, queue, steps, st, &found);
+  cudaError_t e = dispatch_integrate<T>(form, threads, blocks, s, n, p, queue, steps, qs.num_sms, st, &found);
   if (!found) return fail(GRAY2_EINVAL, "gray2_integrate: no compiled variant for %d threads x %d blocks/SM", threads, blocks);
   if (e != cudaSuccess) return fail(GRAY2_ECUDA, "integrate_kernel launch: %s", cudaGetErrorString(e));
 
@@ -199,10 +225,11 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, cons
     CUDA_TRY(cudaMemsetAsync(device_stats, 0, sizeof(gray2_stats), st));
     CUDA_TRY(cudaMemcpyAsync(&device_stats->steps, steps, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st));
     unsigned grid = (unsigned)((n + 255) / 256);
-    if (grid > (unsigned)(g_num_sms * 8)) grid = (unsigned)(g_num_sms * 8);
+    if (grid > (unsigned)(qs.num_sms * 8)) grid = (unsigned)(qs.num_sms * 8);
     gray2::count_status_kernel<<<grid, 256, 0, st>>>(s->status, n, device_stats);
     CUDA_TRY(cudaGetLastError());
   }
+  CUDA_TRY(cudaEventRecord(qs.done, st));      // the slot is free again once this point of `st` is reached
   return GRAY2_OK;
 }
 
@@ -221,8 +248,10 @@ int diag_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_co
   p.r_escape = (T)sc->r_escape;
   p.r_escape_fin = p.r_escape;
   p.lambda_end = lambda_end; p.dir = (double)sc->dir; p.mode = sc->mode; p.max_steps = sc->max_steps; p.clip = 1;
-  unsigned slot = g_queue_next.fetch_add(1) % kQueueSlots;
-  unsigned long long *steps = g_queue + 8 * slot + 1;
+  QueueSlot qs;
+  int rc = acquire_slot(st, &qs);
+  if (rc) return rc;
+  unsigned long long *steps = qs.steps;
   CUDA_TRY(cudaMemsetAsync(steps, 0, sizeof(unsigned long long), st));
   gray2::DiagView out{d->max_abs_u2, d->cos_peak, d->dphi_cycle, d->t_zmax1, d->t_zmax2};
   double mu2 = s->kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
@@ -234,10 +263,11 @@ int diag_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_co
     CUDA_TRY(cudaMemsetAsync(device_stats, 0, sizeof(gray2_stats), st));
     CUDA_TRY(cudaMemcpyAsync(&device_stats->steps, steps, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st));
     unsigned g2 = (unsigned)((n + 255) / 256);
-    if (g2 > (unsigned)(g_num_sms * 8)) g2 = (unsigned)(g_num_sms * 8);
+    if (g2 > (unsigned)(qs.num_sms * 8)) g2 = (unsigned)(qs.num_sms * 8);
     gray2::count_status_kernel<<<g2, 256, 0, st>>>(s->status, n, device_stats);
     CUDA_TRY(cudaGetLastError());
   }
+  CUDA_TRY(cudaEventRecord(qs.done, st));
   return GRAY2_OK;
 }
 
@@ -375,8 +405,6 @@ static int integrate_common(int form, const char *who, gray2_state *s, uint64_t 
     if (form != 0) return fail(GRAY2_EINVAL, "%s: needs a Kerr-Schild state (s->coords = GRAY2_KS)", who);
     form = 2;
   }
-  rc = ensure_scratch();
-  if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   return prec == GRAY2_F64 ? integrate_impl<double>(form, s, n, end, sc, device_stats, st)
                            : integrate_impl<float>(form, s, n, end, sc, device_stats, st);
@@ -411,8 +439,6 @@ int gray2_integrate_diagnostics(gray2_state *s, uint64_t n, double lambda_end, c
   if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(lambda_end) || sc->max_steps < 0)
     return fail(GRAY2_EINVAL, "%s: bad capture_factor / r_escape / lambda_end / max_steps", who);
   if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a_eff| must be <= 1", who);
-  rc = ensure_scratch();
-  if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   return prec == GRAY2_F64 ? diag_impl<double>(s, n, lambda_end, sc, diag, device_stats, st)
                            : diag_impl<float>(s, n, lambda_end, sc, diag, device_stats, st);

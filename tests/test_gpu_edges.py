@@ -159,6 +159,28 @@ def test_concurrent_calls_on_two_streams():
         assert torch.equal(q, g.q) and torch.equal(ns, g.nsteps) and gray2.stats_dict(st) == sd
 
 
+def test_more_calls_in_flight_than_work_queue_slots():
+    """The library has 64 work-queue slots per device.  160 integrations enqueued without a synchronise on
+    four streams (slots are reused while earlier users may still run: the reuse waits on the device) give the
+    bits of the same image integrated alone."""
+    cfg = inputs.CFG3_NULL.scaled(48)
+    _, ref, ref_stats = run_gpu_image(cfg)
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    runs = []
+    torch.cuda.synchronize()
+    for i in range(160):
+        stream = streams[i % 4]
+        with torch.cuda.stream(stream):
+            g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, stream=stream)
+            st = gray2.new_stats()
+            gray2.integrate(g, INF, image_sc(cfg)[0], stats=st, stream=stream)
+            runs.append((g, st))
+    torch.cuda.synchronize()
+    for g, st in runs:
+        assert torch.equal(ref.q, g.q) and torch.equal(ref.nsteps, g.nsteps) and torch.equal(ref.status, g.status)
+        assert gray2.stats_dict(st) == ref_stats
+
+
 def test_backward_direction_and_lambda_clip():
     xu8, _ = inputs.cfg4_ensemble(64)
     g = gray2.init_timelike(0.7, xu8)
