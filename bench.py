@@ -332,7 +332,7 @@ def run_gpu(args):
     scratch = torch.zeros(8, dtype=torch.float64 if prec == gray2.F64 else torch.float32, device="cuda")
     iters = 20000 if prec == gray2.F64 else 40000
     probe = {}
-    for name, regs in (("imm", False), ("regs", True)):
+    for name, regs in (("imm", 0), ("regs", 1), ("fresh", 2)) + ((("packed", 3),) if prec == gray2.F32 else ()):
         gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch, register_operands=regs)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -374,7 +374,9 @@ def run_gpu(args):
                          "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,
                          "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (n_sms, FP_LANES[args.dtype], sm_max_mhz),
                          "fma_probe_tflops": fma_probe_tflops, "frac_of_fma_probe": achieved / fma_probe_tflops,
-                         "fma_probe_register_operands_tflops": probe["regs"]},
+                         "fma_probe_register_operands_tflops": probe["regs"],
+                         "fma_probe_fresh_register_operands_tflops": probe["fresh"],
+                         "fma_probe_packed_fp32x2_tflops": probe.get("packed")},
         }
         if not args.no_cpu_baseline and world == 1:
             # a first pass on oracle_side^2 rays sizes the sample: about 12 s of wall clock on this box's cores

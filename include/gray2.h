@@ -216,8 +216,11 @@ int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void
 
 /* Diagnostic entry: FMA-only probe kernel (8 independent chains per thread) for measuring the attainable
  * FMA rate of the FP64 / FP32 pipe.  register_operands = 0: multiplier and addend are immediates (best
- * case of the pipe); 1: three per-thread register operands (what real code issues; bounded by register-file
- * read bandwidth).  scratch: DEVICE pointer, >= 1 element.  Flops = 16*iters*blocks*threads. */
+ * case of the pipe); 1: three per-thread register operands, multiplier and addend shared by the chains;
+ * 2: every chain has its own multiplier and addend, three fresh register reads per FMA (what real code
+ * issues; bounded by register-file read bandwidth); 3 (GRAY2_F32 only): as 2, made of the packed FFMA2
+ * instruction of the default FP32 integrator.  scratch: DEVICE pointer, >= 1 element.
+ * Flops = 16*iters*blocks*threads (32*iters*blocks*threads for the packed probe). */
 int gray2_fma_probe(int32_t prec, int32_t register_operands, int32_t blocks, int32_t threads, int32_t iters,
                     void *scratch, void *cuda_stream);
 

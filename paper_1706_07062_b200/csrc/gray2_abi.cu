@@ -551,19 +551,30 @@ int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 566 : 598
 
 /* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
  * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
- * register_operands = 0: multiplier and addend are immediates; 1: three per-thread register operands.
+ * register_operands = 0: multiplier and addend are immediates; 1: three per-thread register operands, two of
+ * them shared by the chains; 2: three register operands per FMA, none shared with the neighbouring FMAs;
+ * 3 (GRAY2_F32 only): as 2 with the packed FFMA2 instruction, two floats per operand, flops = 32*iters*blocks*threads.
  * scratch: DEVICE pointer to at least one element of the precision's type.  Flops = 16*iters*blocks*threads. */
 int gray2_fma_probe(int32_t prec, int32_t register_operands, int32_t blocks, int32_t threads, int32_t iters,
                     void *scratch, void *cuda_stream) {
   if (!scratch || blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0)
     return fail(GRAY2_EINVAL, "gray2_fma_probe: bad argument");
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (register_operands == 3) {
+    if (prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_fma_probe: the packed probe (3) exists for GRAY2_F32 only");
+    gray2::fma2_probe_kernel<<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+    CUDA_TRY(cudaGetLastError());
+    return GRAY2_OK;
+  }
+  if (register_operands < 0 || register_operands > 3) return fail(GRAY2_EINVAL, "gray2_fma_probe: register_operands must be 0, 1, 2 or 3");
   if (prec == GRAY2_F64) {
-    if (register_operands) gray2::fma_probe_kernel<double, true><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
-    else gray2::fma_probe_kernel<double, false><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
+    if (register_operands == 2) gray2::fma_probe_kernel<double, 2><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
+    else if (register_operands) gray2::fma_probe_kernel<double, 1><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
+    else gray2::fma_probe_kernel<double, 0><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
   } else if (prec == GRAY2_F32) {
-    if (register_operands) gray2::fma_probe_kernel<float, true><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
-    else gray2::fma_probe_kernel<float, false><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+    if (register_operands == 2) gray2::fma_probe_kernel<float, 2><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+    else if (register_operands) gray2::fma_probe_kernel<float, 1><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
+    else gray2::fma_probe_kernel<float, 0><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
   } else return fail(GRAY2_EINVAL, "gray2_fma_probe: unknown precision");
   CUDA_TRY(cudaGetLastError());
   return GRAY2_OK;

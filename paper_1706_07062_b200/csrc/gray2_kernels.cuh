@@ -592,22 +592,59 @@ __global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos
 
 // Diagnostic: FMA-only probe of the FP64 / FP32 pipe (8 independent chains per thread, registers only).
 // Each thread executes 8 * iters FMAs; the launch's flop count is 2 * 8 * iters * threads.
-// REGS = false: multiplier and addend are immediates (the pipe's best case);
-// REGS = true : all three operands are registers that differ per thread, as in real code, which on
-//               B200 is limited by register-file read bandwidth rather than by the pipe.
-template <typename T, bool REGS>
+// REGS = 0: multiplier and addend are immediates (the pipe's best case);
+// REGS = 1: all three operands are registers that differ per thread, multiplier and addend shared by the
+//           eight chains (consecutive instructions find two of their operands in the operand-reuse cache);
+// REGS = 2: every chain has its own multiplier and addend, so that no instruction shares a source register
+//           with its neighbours -- three fresh register reads per FMA, the mix real code issues, which on
+//           B200 is limited by register-file read bandwidth rather than by the pipe.
+template <typename T, int REGS>
 __global__ void fma_probe_kernel(int iters, T seed, T *__restrict__ out) {
   T a0 = seed + T(threadIdx.x), a1 = a0 + T(1), a2 = a0 + T(2), a3 = a0 + T(3);
   T a4 = a0 + T(4), a5 = a0 + T(5), a6 = a0 + T(6), a7 = a0 + T(7);
-  const T m = REGS ? T(0.999999) + T(threadIdx.x) * T(1e-9) : T(0.999999);
-  const T c = REGS ? T(1e-6) + T(threadIdx.x) * T(1e-9) : T(1e-6);
+  if constexpr (REGS == 2) {
+    const T d = T(threadIdx.x) * T(1e-9);
+    const T m0 = T(0.999999) + d, m1 = T(0.999998) + d, m2 = T(0.999997) + d, m3 = T(0.999996) + d;
+    const T m4 = T(0.999995) + d, m5 = T(0.999994) + d, m6 = T(0.999993) + d, m7 = T(0.999992) + d;
+    const T c0 = T(1e-6) + d, c1 = T(2e-6) + d, c2 = T(3e-6) + d, c3 = T(4e-6) + d;
+    const T c4 = T(5e-6) + d, c5 = T(6e-6) + d, c6 = T(7e-6) + d, c7 = T(8e-6) + d;
 #pragma unroll 8
-  for (int i = 0; i < iters; ++i) {
-    a0 = fma_(a0, m, c); a1 = fma_(a1, m, c); a2 = fma_(a2, m, c); a3 = fma_(a3, m, c);
-    a4 = fma_(a4, m, c); a5 = fma_(a5, m, c); a6 = fma_(a6, m, c); a7 = fma_(a7, m, c);
+    for (int i = 0; i < iters; ++i) {
+      a0 = fma_(a0, m0, c0); a1 = fma_(a1, m1, c1); a2 = fma_(a2, m2, c2); a3 = fma_(a3, m3, c3);
+      a4 = fma_(a4, m4, c4); a5 = fma_(a5, m5, c5); a6 = fma_(a6, m6, c6); a7 = fma_(a7, m7, c7);
+    }
+  } else {
+    const T m = REGS ? T(0.999999) + T(threadIdx.x) * T(1e-9) : T(0.999999);
+    const T c = REGS ? T(1e-6) + T(threadIdx.x) * T(1e-9) : T(1e-6);
+#pragma unroll 8
+    for (int i = 0; i < iters; ++i) {
+      a0 = fma_(a0, m, c); a1 = fma_(a1, m, c); a2 = fma_(a2, m, c); a3 = fma_(a3, m, c);
+      a4 = fma_(a4, m, c); a5 = fma_(a5, m, c); a6 = fma_(a6, m, c); a7 = fma_(a7, m, c);
+    }
   }
   T s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
   if (s == T(-12345.678)) out[0] = s;   // never true; keeps the chains alive
+}
+
+// The same for the packed FP32x2 instruction (FFMA2) that the default FP32 integrator is made of: eight chains
+// of float pairs per thread, every chain with its own multiplier and addend pair (three fresh 64-bit register
+// reads per instruction).  Flops = 2 * 2 * 8 * iters * threads.
+__global__ void fma2_probe_kernel(int iters, float seed, float *__restrict__ out) {
+  const float b = seed + (float)threadIdx.x, d = (float)threadIdx.x * 1e-9f;
+  f32x2 a[8], m[8], c[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    a[j] = f32x2(b + (float)j, b + (float)j + 0.5f);
+    m[j] = f32x2(0.999999f - (float)j * 1e-6f + d, 0.999991f - (float)j * 1e-6f + d);
+    c[j] = f32x2((float)(j + 1) * 1e-6f + d, (float)(j + 1) * 1.5e-6f + d);
+  }
+#pragma unroll 8
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a[j] = fma_(a[j], m[j], c[j]);
+  }
+  f32x2 s = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
+  if (s.v.x + s.v.y == -12345.678f) out[0] = s.v.x;   // never true; keeps the chains alive
 }
 
 __global__ void count_status_kernel(const int32_t *__restrict__ status, uint64_t n, gray2_stats *stats) {

@@ -284,11 +284,12 @@ def convert(st: State, to_coords: int, n=None, stream=None, out: State | None = 
 
 
 def fma_probe(prec, blocks, threads, iters, scratch: torch.Tensor, register_operands=False, stream=None):
-    """Diagnostic: enqueue the FMA-only probe kernel; flops = 16 * iters * blocks * threads."""
+    """Diagnostic: enqueue the FMA-only probe kernel; returns its flops, 16 * iters * blocks * threads
+    (twice that for register_operands = 3, the packed FP32x2 probe)."""
     _check(load_library().gray2_fma_probe(prec, int(register_operands), blocks, threads, iters,
                                           C.c_void_p(scratch.data_ptr()),
                                           _stream_ptr(stream)))
-    return 16 * iters * blocks * threads
+    return (32 if int(register_operands) == 3 else 16) * iters * blocks * threads
 
 
 def set_launch(prec, threads_per_block=0, blocks_per_sm=0):

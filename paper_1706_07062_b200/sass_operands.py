@@ -1,0 +1,123 @@
+"""Register-operand accounting of the integrator's hot loop, read from the SASS of the built library.
+
+    python -m paper_1706_07062_b200.sass_operands [path/to/libgray2.so] [substring of the kernel name]
+
+Why.  On B200 an FP64 (or packed FP32x2) arithmetic warp instruction occupies its pipe for two cycles, but
+the register file delivers one 64-bit operand per cycle and sub-partition: measured with
+`gray2_fma_probe`, an FMA whose three source registers are all different and none of
+which the previous instruction left in the operand-reuse cache takes THREE cycles, while an instruction with
+at most two such operands (a multiply, an add, an FMA with an immediate, a uniform register, the same
+register twice, or a `.reuse` hit) takes two.  The cost of the loop is therefore
+
+    cycles per warp-step  =  sum over its FP instructions of max(2, distinct fresh register operands),
+
+not twice the instruction count.  This tool applies that model to the inner loop of every
+`integrate_kernel*` in the library, so that a change of the arithmetic can be judged before it is timed.
+
+It is a development aid: nothing on the product path imports it.  Needs `cuobjdump` (CUDA toolkit).
+"""
+from __future__ import annotations
+
+import os
+import re
+import subprocess
+import sys
+
+FP_OPS = ("DFMA", "DMUL", "DADD", "FFMA2", "FMUL2", "FADD2")
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _instructions(function_text: str):
+    out = []
+    for line in function_text.split("\n"):
+        m = re.match(r"\s*/\*([0-9a-f]{4,})\*/\s+(.*?);", line)
+        if m:
+            out.append((int(m.group(1), 16), m.group(2).strip()))
+    return out
+
+
+def _inner_loop(ins):
+    """The smallest backward-branch span that holds more than 250 FP instructions: the RK4 step loop."""
+    spans = []
+    for addr, text in ins:
+        m = re.search(r"BRA 0x([0-9a-f]+)", text)
+        if m and int(m.group(1), 16) < addr:
+            lo = int(m.group(1), 16)
+            body = [t for a, t in ins if lo <= a <= addr]
+            nfp = sum(1 for t in body if _opcode(t).startswith(FP_OPS))
+            if nfp > 250:
+                spans.append((len(body), lo, addr))
+    if not spans:
+        return []
+    _, lo, hi = min(spans)
+    return [(a, t) for a, t in ins if lo <= a <= hi]
+
+
+def _opcode(text: str) -> str:
+    if text.startswith("@"):
+        text = text.split(None, 1)[1]
+    return text.split()[0]
+
+
+def account(loop):
+    """Returns a dict with the counts of the model for one loop body."""
+    reuse_prev = {}
+    res = {"instructions": len(loop), "fp": 0, "cycles": 0, "three_read": 0, "reuse_hits": 0, "by_op": {}}
+    for _, text in loop:
+        if text.startswith("@"):
+            text = text.split(None, 1)[1]
+        op = text.split()[0]
+        srcs = [x.strip() for x in text[len(op):].split(",")][1:]
+        is_fp = op.startswith(FP_OPS)
+        fresh, reuse_now = set(), {}
+        for slot, s in enumerate(srcs):
+            s = s.lstrip("-|~!").rstrip("|")
+            if s.startswith("R") and not s.startswith("RZ"):
+                reg = s.split(".")[0]
+                if is_fp:
+                    if reuse_prev.get(slot) == reg:
+                        res["reuse_hits"] += 1
+                    else:
+                        fresh.add(reg)
+                if ".reuse" in s:
+                    reuse_now[slot] = reg
+        reuse_prev = reuse_now
+        if is_fp:
+            base = op.split(".")[0]
+            res["by_op"][base] = res["by_op"].get(base, 0) + 1
+            res["fp"] += 1
+            res["cycles"] += max(2, len(fresh))
+            res["three_read"] += len(fresh) == 3
+    return res
+
+
+def report(lib: str, name_filter: str = "integrate_kernel"):
+    txt = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
+    rows = []
+    for fn in re.split(r"\n\s*Function : ", txt)[1:]:
+        name = fn.split("\n", 1)[0].strip()
+        if name_filter not in name:
+            continue
+        loop = _inner_loop(_instructions(fn))
+        if loop:
+            rows.append((name, account(loop)))
+    return rows
+
+
+def main(argv):
+    lib = argv[1] if len(argv) > 1 else os.path.join(HERE, "libgray2.so")
+    filt = argv[2] if len(argv) > 2 else "integrate_kernel"
+    demangle = subprocess.run(["c++filt"], input="\n".join(n for n, _ in report(lib, filt)), capture_output=True, text=True)
+    names = demangle.stdout.split("\n") if demangle.returncode == 0 else None
+    for i, (name, r) in enumerate(report(lib, filt)):
+        shown = names[i] if names else name
+        shown = re.sub(r"\(.*", "", shown)
+        ops = " ".join("%s %d" % kv for kv in sorted(r["by_op"].items()))
+        print("%s\n    loop: %d instructions, %d FP (%s); three-read FP instructions %d, reuse hits %d\n"
+              "    pipe cycles 2 x FP = %d ; operand-model cycles = %d  (%.3f of them pipe)" %
+              (shown, r["instructions"], r["fp"], ops, r["three_read"], r["reuse_hits"], 2 * r["fp"], r["cycles"],
+               2 * r["fp"] / r["cycles"]))
+
+
+if __name__ == "__main__":
+    main(sys.argv)
