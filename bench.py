@@ -410,8 +410,8 @@ def main():
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--blocks", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--e2e-chunks", type=int, default=8, help="end-to-end leg: chunks pipelined over the streams")
-    ap.add_argument("--e2e-streams", type=int, default=2, help="end-to-end leg: number of streams the chunks alternate between")
+    ap.add_argument("--e2e-chunks", type=int, default=32, help="end-to-end leg: chunks pipelined over the streams")
+    ap.add_argument("--e2e-streams", type=int, default=8, help="end-to-end leg: number of streams the chunks alternate between")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
