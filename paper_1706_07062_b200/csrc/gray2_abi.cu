@@ -187,24 +187,30 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
   return cudaSuccess;
 }
 
+// Step parameters of the kernels from the caller's step control (`end` = lambda_end or t_end).
 template <typename T>
-int integrate_impl(int form, gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
-                   gray2_stats *device_stats, cudaStream_t st) {
-  const double a = s->a_eff;
+gray2::StepParams<T> make_params(double a, double end, const gray2_step_control *sc, bool always_clip) {
   gray2::StepParams<T> p;
   p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a); p.k.four_a2 = (T)(4.0 * a * a);
   p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
   p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
   p.r_escape = (T)sc->r_escape;
-  {
-    const double big = sizeof(T) == 8 ? 1.7976931348623157e308 : 3.402823466e38;
-    p.r_escape_fin = (T)(sc->r_escape < big ? sc->r_escape : big);
-  }
-  p.lambda_end = lambda_end;
+  // the hot loop tests r <= r_escape_fin with r_escape_fin finite, so that r = inf fails the test too
+  const double big = sizeof(T) == 8 ? 1.7976931348623157e308 : 3.402823466e38;
+  p.r_escape_fin = always_clip ? p.r_escape : (T)(sc->r_escape < big ? sc->r_escape : big);
+  p.lambda_end = end;
   p.dir = (double)sc->dir;
   p.mode = sc->mode;
   p.max_steps = sc->max_steps;
-  p.clip = !(isinf(lambda_end) && (double)sc->dir * lambda_end > 0.0);
+  // clip = 0 only when dir * end = +inf: the end test can never fire and the last step never needs clipping
+  p.clip = always_clip || !(isinf(end) && (double)sc->dir * end > 0.0);
+  return p;
+}
+
+template <typename T>
+int integrate_impl(int form, gray2_state *s, uint64_t n, double end, const gray2_step_control *sc,
+                   gray2_stats *device_stats, cudaStream_t st) {
+  const gray2::StepParams<T> p = make_params<T>(s->a_eff, end, sc, /*always_clip=*/false);
 
   QueueSlot qs;
   int rc = acquire_slot(st, &qs);
@@ -240,14 +246,8 @@ namespace {
 template <typename T>
 int diag_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_control *sc,
                      const gray2_diagnostics *d, gray2_stats *device_stats, cudaStream_t st) {
-  const double a = s->a_eff;
-  gray2::StepParams<T> p;
-  p.k.a = (T)a; p.k.a2 = (T)(a * a); p.k.two_a = (T)(2.0 * a); p.k.two_a2 = (T)(2.0 * a * a); p.k.four_a2 = (T)(4.0 * a * a);
-  p.eta_or_h = (T)((double)sc->dir * (sc->mode == 1 ? sc->eta : sc->h_fixed));
-  p.r_capture = (T)(sc->capture_factor * (1.0 + sqrt(1.0 - a * a)));
-  p.r_escape = (T)sc->r_escape;
-  p.r_escape_fin = p.r_escape;
-  p.lambda_end = lambda_end; p.dir = (double)sc->dir; p.mode = sc->mode; p.max_steps = sc->max_steps; p.clip = 1;
+  // the diagnostics kernel always tests lambda_end and compares r with r_escape itself
+  const gray2::StepParams<T> p = make_params<T>(s->a_eff, lambda_end, sc, /*always_clip=*/true);
   QueueSlot qs;
   int rc = acquire_slot(st, &qs);
   if (rc) return rc;
@@ -387,10 +387,9 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
   return GRAY2_OK;
 }
 
-static int integrate_common(int form, const char *who, gray2_state *s, uint64_t n, double end,
-                            const gray2_step_control *sc, int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
-  int rc = check_state(s, who);
-  if (rc) return rc;
+// Arguments common to gray2_integrate, gray2_integrate_coordtime and gray2_integrate_diagnostics.
+static int check_integrate_args(const char *who, const gray2_state *s, uint64_t n, double end,
+                                const gray2_step_control *sc, int32_t prec) {
   if (!sc) return fail(GRAY2_EINVAL, "%s: step control is NULL", who);
   if (n == 0) return fail(GRAY2_EINVAL, "%s: n == 0", who);
   if (n > s->n) return fail(GRAY2_ESTATE, "%s: n (%llu) exceeds s->n (%llu)", who, (unsigned long long)n, (unsigned long long)s->n);
@@ -401,6 +400,15 @@ static int integrate_common(int form, const char *who, gray2_state *s, uint64_t 
   if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(end) || sc->max_steps < 0)
     return fail(GRAY2_EINVAL, "%s: bad capture_factor / r_escape / end value / max_steps", who);
   if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a_eff| must be <= 1", who);
+  return GRAY2_OK;
+}
+
+static int integrate_common(int form, const char *who, gray2_state *s, uint64_t n, double end,
+                            const gray2_step_control *sc, int32_t prec, gray2_stats *device_stats, void *cuda_stream) {
+  int rc = check_state(s, who);
+  if (rc) return rc;
+  rc = check_integrate_args(who, s, n, end, sc, prec);
+  if (rc) return rc;
   if (s->coords == GRAY2_BL) {
     if (form != 0) return fail(GRAY2_EINVAL, "%s: needs a Kerr-Schild state (s->coords = GRAY2_KS)", who);
     form = 2;
@@ -430,15 +438,8 @@ int gray2_integrate_diagnostics(gray2_state *s, uint64_t n, double lambda_end, c
   if (s->coords != GRAY2_KS) return fail(GRAY2_EINVAL, "%s: needs a Kerr-Schild state (s->coords = GRAY2_KS)", who);
   if (!diag->max_abs_u2 || !diag->cos_peak || !diag->dphi_cycle || !diag->t_zmax1 || !diag->t_zmax2)
     return fail(GRAY2_EINVAL, "%s: a diagnostics array is NULL", who);
-  if (n == 0) return fail(GRAY2_EINVAL, "%s: n == 0", who);
-  if (n > s->n) return fail(GRAY2_ESTATE, "%s: n exceeds s->n", who);
-  if (prec != s->prec) return fail(GRAY2_EINVAL, "%s: prec differs from s->prec", who);
-  if (sc->mode != 0 && sc->mode != 1) return fail(GRAY2_EINVAL, "%s: mode must be 0 or 1", who);
-  if (sc->mode == 1 ? !(sc->eta > 0.0) : !(sc->h_fixed > 0.0)) return fail(GRAY2_EINVAL, "%s: step size must be > 0", who);
-  if (sc->dir != 1 && sc->dir != -1) return fail(GRAY2_EINVAL, "%s: dir must be +1 or -1", who);
-  if (!(sc->capture_factor > 0.0) || isnan(sc->r_escape) || isnan(lambda_end) || sc->max_steps < 0)
-    return fail(GRAY2_EINVAL, "%s: bad capture_factor / r_escape / lambda_end / max_steps", who);
-  if (!(fabs(s->a_eff) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a_eff| must be <= 1", who);
+  rc = check_integrate_args(who, s, n, lambda_end, sc, prec);
+  if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   return prec == GRAY2_F64 ? diag_impl<double>(s, n, lambda_end, sc, diag, device_stats, st)
                            : diag_impl<float>(s, n, lambda_end, sc, diag, device_stats, st);
