@@ -129,6 +129,29 @@ def test_new_entries_reject_bad_arguments_without_gpu_work(lib):
     assert lib.gray2_rhs_bl(0, 0.5, 0, null, null, null, null) == EINVAL
     assert lib.gray2_flops_per_step_bl(0) == 598 and lib.gray2_flops_per_step_bl(1) == 566
     assert lib.gray2_flops_per_step_coordtime(0) == 534
+    fake = C.c_void_p(0x1000)
+    assert lib.gray2_fma_probe(0, 7, 1, 32, 1, fake, null) == EINVAL                  # unknown operand form
+    assert lib.gray2_fma_probe(0, 3, 1, 32, 1, fake, null) == EINVAL                  # packed form is FP32 only
+    assert lib.gray2_fma_probe(1, 2, 1, 32, 1, null, null) == EINVAL                  # no scratch
+
+
+def test_sass_operand_model_on_a_hand_written_loop():
+    """The cost model of paper_1706_07062_b200.sass_operands: max(2, distinct fresh register
+    operands) cycles per FP64 / packed FP32x2 instruction; immediates, uniform registers, a register named twice
+    and a `.reuse` hit of the previous instruction are free."""
+    from paper_1706_07062_b200 import sass_operands as so
+    loop = [(0x00, "DFMA R0, R2, R4, R6"),            # three fresh registers: 3
+            (0x10, "DMUL R8, R2, R4"),                # two: 2
+            (0x20, "DFMA R10, R12, R12, 1"),          # one register named twice and an immediate: 2 (floor)
+            (0x30, "DFMA R14, R16.reuse, R18, R20"),  # 3, leaves R16 in slot 0
+            (0x40, "DFMA R22, R16, R24, R26"),        # R16 comes from the reuse cache: 2
+            (0x50, "IMAD.MOV.U32 R30, RZ, RZ, RZ"),   # not an FP instruction, breaks nothing it did not set
+            (0x60, "DFMA R22, R16, R24, UR4"),        # uniform register: 2
+            (0x70, "@P0 DADD R2, R2, -R6")]           # predicated add: 2
+    r = so.account(loop)
+    assert r["fp"] == 7 and r["cycles"] == 3 + 2 + 2 + 3 + 2 + 2 + 2
+    assert r["three_read"] == 2 and r["reuse_hits"] == 1
+    assert r["by_op"] == {"DFMA": 5, "DMUL": 1, "DADD": 1}
 
 
 def test_bench_reference_arm_prints_the_contract_line():

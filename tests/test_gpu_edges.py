@@ -181,6 +181,19 @@ def test_more_calls_in_flight_than_work_queue_slots():
         assert gray2.stats_dict(st) == ref_stats
 
 
+def test_fma_probes_run_in_every_form():
+    """The diagnostic FMA kernels behind bench.py's fma_probe_* fields: every operand form launches and
+    reports its flop count (16 per thread and iteration, 32 for the packed FP32x2 form)."""
+    for prec, dtype, forms in ((gray2.F64, torch.float64, (0, 1, 2)), (gray2.F32, torch.float32, (0, 1, 2, 3))):
+        scratch = torch.zeros(8, dtype=dtype, device="cuda")
+        for form in forms:
+            flops = gray2.fma_probe(prec, 4, 64, 10, scratch, register_operands=form)
+            assert flops == (32 if form == 3 else 16) * 10 * 4 * 64
+    torch.cuda.synchronize()
+    with pytest.raises(Exception):
+        gray2.fma_probe(gray2.F64, 4, 64, 10, torch.zeros(8, dtype=torch.float64, device="cuda"), register_operands=3)
+
+
 def test_backward_direction_and_lambda_clip():
     xu8, _ = inputs.cfg4_ensemble(64)
     g = gray2.init_timelike(0.7, xu8)
