@@ -89,6 +89,7 @@ def lib():
         _lib.oracle_bl_trajectory.argtypes = [d, p, d, C.c_int64, C.c_int64, p]
         _lib.oracle_init_null.argtypes = [p, d, d, d, d, d, C.c_int32, C.c_int32]
         _lib.oracle_init_timelike.argtypes = [p, d, p, C.c_uint64, C.c_int32]
+        _lib.oracle_init_explicit.argtypes = [p, d, p, C.c_uint64, C.c_int32, C.c_int32]
         _lib.oracle_integrate.argtypes = [p, C.c_uint64, d, p, p]
         _lib.oracle_invariants.argtypes = [p, C.c_uint64, p, p, p, p]
         _lib.oracle_ks_coordtime_accel.argtypes = [d, p, p, p]
@@ -178,6 +179,18 @@ def init_timelike(a, xu8, renormalise_ut=False) -> State:
     rc = lib().oracle_init_timelike(C.byref(cs), a, _ptr(xu8), xu8.shape[0], int(renormalise_ut))
     if rc:
         raise ValueError("oracle_init_timelike: invalid arguments")
+    st._back(cs)
+    return st
+
+
+def init_explicit(a, xu8, kind=NULL, renormalise_ut=False) -> State:
+    """Explicit 8-vectors of null (Table 1) or time-like geodesics."""
+    xu8 = np.ascontiguousarray(np.asarray(xu8, dtype=np.float64).reshape(-1, 8))
+    st = State(xu8.shape[0])
+    cs = st._c()
+    rc = lib().oracle_init_explicit(C.byref(cs), a, _ptr(xu8), xu8.shape[0], int(kind), int(renormalise_ut))
+    if rc:
+        raise ValueError("oracle_init_explicit: invalid arguments")
     st._back(cs)
     return st
 

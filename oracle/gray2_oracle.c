@@ -307,18 +307,27 @@ int oracle_init_null(oracle_state *s, double a, double r_obs, double inc,
   return 0;
 }
 
-/* Explicit 8-vectors ("8 variables"; PAPER.md:263 explicit v_z kick).  xu8 is AoS n x 8.
- * renormalise_ut != 0 re-solves u^t from g u u = -1 (DESIGN R7). */
-int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renorm)
+/* Explicit 8-vectors ("8 variables") of either kind: the paper's convergence experiments start
+ * from explicit data for photons (the spherical photon orbits of Table 1) and
+ * for particles (the circular orbits with the v_z kick).  xu8 is AoS n x 8.
+ * kind: ORACLE_NULL (mu^2 = 0) or ORACLE_TIMELIKE (mu^2 = 1); it is recorded in the state (Carter's Q uses
+ * it, DESIGN R8) and renormalise_ut != 0 re-solves u^t from g u u = -mu^2 (DESIGN R7). */
+int oracle_init_explicit(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t kind, int32_t renorm)
 {
   if (!s || !xu8 || n == 0 || n > s->n || !(fabs(a) <= 1.0)) return 1;
-  s->a_eff = a; s->kind = ORACLE_TIMELIKE; s->reversed = 0; s->coords = ORACLE_KS;
+  if (kind != ORACLE_NULL && kind != ORACLE_TIMELIKE) return 1;
+  s->a_eff = a; s->kind = kind; s->reversed = 0; s->coords = ORACLE_KS;
   for (uint64_t k = 0; k < n; ++k) {
     for (int m = 0; m < 8; ++m) s->q[m][k] = xu8[k * 8 + m];
-    if (renorm) s->q[4][k] = solve_ut(a, &xu8[k * 8 + 1], &xu8[k * 8 + 5], 1.0);
+    if (renorm) s->q[4][k] = solve_ut(a, &xu8[k * 8 + 1], &xu8[k * 8 + 5], kind == ORACLE_TIMELIKE ? 1.0 : 0.0);
     s->lambda[k] = 0.0; s->status[k] = ORACLE_ACTIVE; s->nsteps[k] = 0;
   }
   return 0;
+}
+
+int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renorm)
+{
+  return oracle_init_explicit(s, a, xu8, n, ORACLE_TIMELIKE, renorm);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -346,12 +355,15 @@ static void integrate_one(double a, int32_t coords, double y[8], double *lambda,
     if (*nsteps >= sc->max_steps)        { *status = ORACLE_MAXSTEPS; break; }
     if (dir * (lambda_end - *lambda) <= 0.0) break; /* stays ACTIVE: resumable */
     double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
-    if (fabs(h) > fabs(lambda_end - *lambda)) h = lambda_end - *lambda; /* clip the last step */
+    /* clip the last step; the clock then lands on lambda_end itself, not on lambda + (lambda_end - lambda),
+       which may differ from it by an ulp and would cost one more, ulp-sized, step (DESIGN R22) */
+    int clipped = fabs(h) > fabs(lambda_end - *lambda);
+    if (clipped) h = lambda_end - *lambda;
     if (coords == ORACLE_BL) {
       /* a stage at r < capture radius: CAPTURED at the state before this step (DESIGN R20) */
       if (oracle_bl_rk4_step_guarded(a, y, h, sc->capture_factor * r_plus)) { *status = ORACLE_CAPTURED; break; }
     } else oracle_rk4_step(a, y, h);
-    *lambda += h;
+    *lambda = clipped ? lambda_end : *lambda + h;
     *nsteps += 1;
   }
 }
@@ -456,9 +468,10 @@ int oracle_integrate_coordtime(oracle_state *s, uint64_t n, double t_end,
         if (ns >= sc->max_steps) { st = ORACLE_MAXSTEPS; break; }
         if (dir * (t_end - t) <= 0.0) break;
         double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
-        if (fabs(h) > fabs(t_end - t)) h = t_end - t;
+        int clipped = fabs(h) > fabs(t_end - t);            /* DESIGN R22: land on t_end itself */
+        if (clipped) h = t_end - t;
         oracle_rk4_step_coordtime(a, y, h);
-        t += h;
+        t = clipped ? t_end : t + h;
         ns += 1;
       }
       s->q[0][k] = t;
@@ -522,7 +535,7 @@ static void diag_sample(diag_acc *D, double a, int32_t kind, const double y[8])
       D->peak = y1 - (y2 - y0) * (y2 - y0) / (8.0 * (y0 - 2.0 * y1 + y2));
       D->have_peak = 1;
     }
-    if (!D->have_dphi && D->k >= 2 && D->zprev < 0.0 && y[3] >= 0.0) {
+    if (!D->have_dphi && D->zprev < 0.0 && y[3] >= 0.0) {     /* k >= 1 here: the pair (z_0, z_1) counts */
       double w = -D->zprev / (y[3] - D->zprev);
       D->dphi = D->phiunf + w * (phiunf - D->phiunf) - D->phi0;
       D->have_dphi = 1;
@@ -564,9 +577,10 @@ int oracle_integrate_diagnostics(oracle_state *s, uint64_t n, double lambda_end,
       if (ns >= sc->max_steps) { st = ORACLE_MAXSTEPS; break; }
       if (dir * (lambda_end - lam) <= 0.0) break;
       double h = dir * (sc->mode == 1 ? sc->eta * r : sc->h_fixed);
-      if (fabs(h) > fabs(lambda_end - lam)) h = lambda_end - lam;
+      int clipped = fabs(h) > fabs(lambda_end - lam);     /* DESIGN R22: land on lambda_end itself */
+      if (clipped) h = lambda_end - lam;
       oracle_rk4_step(a, y, h);
-      lam += h;
+      lam = clipped ? lambda_end : lam + h;
       ns += 1;
     }
     for (int m = 0; m < 8; ++m) s->q[m][k] = y[m];

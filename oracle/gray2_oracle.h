@@ -57,7 +57,8 @@ typedef struct { uint64_t steps, n_captured, n_escaped, n_maxsteps, n_invalid, n
 /* ---- the four operations of the boundary, on host arrays ---- */
 int oracle_init_null(oracle_state *s, double a, double r_obs, double inclination_rad,
                      double fov_half_alpha, double fov_half_beta, int32_t nx, int32_t ny);
-int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renormalise_ut);
+int oracle_init_explicit(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t kind, int32_t renormalise_ut);
+int oracle_init_timelike(oracle_state *s, double a, const double *xu8, uint64_t n, int32_t renormalise_ut);  /* kind = TIMELIKE */
 int oracle_integrate(oracle_state *s, uint64_t n, double lambda_end,
                      const oracle_step_control *sc, oracle_stats *stats /* may be NULL */);
 int oracle_invariants(const oracle_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm);

@@ -325,3 +325,34 @@ def test_bl_stopping_rules_and_resume():
     ab = oracle.convert(axis, oracle.BL)
     st = oracle.integrate(ab, float("inf"), sc)
     assert ab.status[0] == oracle.INVALID and st["steps"] == 0
+
+
+@pytest.mark.parametrize("eta", [0.005, 0.01, 0.02])
+@pytest.mark.parametrize("factor", [1.005, 1.01, 1.02, 1.05])
+def test_guarded_bl_capture_agrees_with_the_unguarded_kerr_schild_run(factor, eta):
+    """The choice of DESIGN R20 (reject a BL step one of whose stages lies inside the capture radius) pinned by
+    something that has no such rule: the Kerr-Schild oracle, whose chart is regular on the horizon
+     and needs no guard, run on the same rays with the same step and capture radius.  The two must
+    agree on which rays are captured, and the BL ray must have been stopped within one step of the radius at
+    which the Kerr-Schild ray stops, never beyond it."""
+    cfg = inputs.CFG3_NULL.scaled(36, 28)
+    k0 = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    sc = oracle.step_control(mode=1, eta=eta, capture_factor=factor, r_escape=cfg.r_escape, max_steps=200000)
+    k1, b1 = k0.copy(), oracle.convert(k0, oracle.BL)
+    oracle.integrate(k1, float("inf"), sc)
+    oracle.integrate(b1, float("inf"), sc)
+    d, mask = ih.classify_image(cfg, k0)
+    use = (d > 2e-2) & (ih.axis_approach(k0) >= 5 * max(eta, 0.01))
+    assert use.mean() > 0.9
+    assert np.array_equal(b1.status[use], k1.status[use])
+    assert np.array_equal((b1.status == oracle.CAPTURED)[use], mask[use])
+    cap = use & (k1.status == oracle.CAPTURED)
+    assert cap.sum() > 40
+    r_cap = factor * cf.r_plus(cfg.a)
+    r_b = b1.q[1][cap]
+    r_k = np.array([oracle.ks_r(k1.a_eff, *k1.q[1:4, j]) for j in np.flatnonzero(cap)])
+    assert (r_k < r_cap).all() and (r_b >= r_cap).all()
+    # |dr/dlambda| <= |P - a xi| / Sigma is a few units next to the horizon: one step h = eta r moves r by < 6 eta r
+    assert (r_b / r_cap - 1.0).max() < 6.0 * eta, (r_b / r_cap - 1.0).max()
+    early = (k1.nsteps - b1.nsteps)[cap]
+    assert early.min() >= 0 and early.max() <= 4 + int(np.ceil(np.log(1.0 + 6.0 * eta) / eta))

@@ -14,8 +14,7 @@ INF = float("inf")
 
 def table1_state():
     xu8 = np.array([cf.spherical_photon_state(1.0, r["r"])[0] for r in ROWS])
-    st = oracle.init_timelike(1.0, xu8)
-    st.kind = oracle.NULL
+    st = oracle.init_explicit(1.0, xu8, oracle.NULL)      # Table 1 are photon orbits given explicitly
     return st, xu8
 
 
@@ -83,3 +82,25 @@ def test_events_that_never_happen_are_nan():
     ref = oracle.init_null(0.5, 50.0, np.radians(90.0), 5.0, 1e-9, 4, 1)
     oracle.integrate(ref, INF, oracle.step_control(mode=1, eta=0.02, r_escape=60.0))
     assert np.array_equal(ref.q, st.q) and np.array_equal(ref.nsteps, st.nsteps) and np.array_equal(ref.status, st.status)
+
+
+def test_upward_zero_between_the_first_two_samples_counts():
+    """gray2.h: dphi_cycle is taken at the first pair z_k < 0 <= z_{k+1}, k = 0, 1, ...  Start Table 1 row A
+    half a step below the equator, moving up: the zero lies between samples 0 and 1.  The expected value is
+    measured on the stored trajectory with numpy (nothing of the accumulator is reused)."""
+    y0, _, _ = cf.spherical_photon_state(1.0, ROWS[0]["r"])
+    h = 1.0 / 64
+    back = oracle.trajectory(1.0, y0, -h, 1)[-1]                   # one step back: z < 0, u^z > 0
+    start = 0.5 * (back + y0)
+    start[4:] = y0[4:]
+    assert start[3] < 0.0 < start[7]
+    st = oracle.init_explicit(1.0, start[None, :], oracle.NULL)
+    _, d = oracle.integrate_diagnostics(st, 2.0, oracle.step_control(mode=0, h_fixed=h, max_steps=10 ** 6))
+    traj = oracle.trajectory(1.0, start, h, 128)
+    z = traj[:, 3]
+    assert z[0] < 0.0 <= z[1]
+    r = np.array([oracle.ks_r(1.0, *p) for p in traj[:, 1:4]])
+    phi = np.unwrap(np.arctan2(traj[:, 2], traj[:, 1]) - np.arctan2(1.0, r))
+    w = -z[0] / (z[1] - z[0])
+    expect = w * (phi[1] - phi[0])
+    assert abs(d["dphi_cycle"][0] - expect) < 1e-13 and 0.0 < expect < 0.05

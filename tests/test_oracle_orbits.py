@@ -5,6 +5,8 @@ import pytest
 
 import closed_forms as cf
 import oracle
+from conftest import load_table1
+from paper_1706_07062_b200 import inputs
 
 INF = float("inf")
 
@@ -33,8 +35,7 @@ def test_schwarzschild_photon_sphere_at_3M():
     for eps, expect in ((-1e-3, oracle.CAPTURED), (+1e-3, oracle.ESCAPED)):
         y = y0.copy()
         y[1] += eps
-        st = oracle.init_timelike(0.0, y[None, :])
-        st.kind = oracle.NULL
+        st = oracle.init_explicit(0.0, y[None, :], oracle.NULL)
         oracle.integrate(st, INF, oracle.step_control(mode=0, h_fixed=1.0 / 32, r_escape=50.0, max_steps=200000))
         assert st.status[0] == expect
 
@@ -272,7 +273,53 @@ def test_circular_photon_orbit_radii_of_eq19_eq20(a):
         scale = (r0 + eps) / r0
         y0[1] *= scale
         y0[2] *= scale
-        st = oracle.init_timelike(a, y0[None, :])
-        st.kind = oracle.NULL
+        st = oracle.init_explicit(a, y0[None, :], oracle.NULL)
         oracle.integrate(st, INF, oracle.step_control(mode=0, h_fixed=1.0 / 64, r_escape=40.0, max_steps=400000))
         assert st.status[0] == expect
+
+
+# ---- explicit initial data of either kind (Table 1: photons; particles) -----
+
+def test_init_explicit_records_the_kind_and_uses_it():
+    """Table 1's spherical photon orbits are explicit NULL data: the state-level invariants must return the
+    paper's (Phi, Q) with mu^2 = 0; declared TIMELIKE the same 8-vector has Q lower by a^2 cos^2(theta) = 0 on
+    the equator but its re-solved u^t differs (g u u = -1 instead of 0)."""
+    a, row = 1.0, load_table1()[4]                    # row E (PAPER.md:180), outside the ergosphere: 1 - f > 0
+    y0, phi, q = cf.spherical_photon_state(a, row["r"])
+    st = oracle.init_explicit(a, y0[None, :], oracle.NULL)
+    assert (st.kind, st.reversed, st.a_eff) == (oracle.NULL, 0, a)
+    E, Lz, Q, norm = oracle.invariants(st)
+    assert abs(E[0] - 1) < 1e-13 and abs(Lz[0] - row["phi"]) < 5e-5 and abs(Q[0] - row["q"]) < 5e-5 and abs(norm[0]) < 1e-13
+    # off the equator mu^2 enters Q: a^2 cos^2(theta) (mu^2 - E^2)
+    tr = oracle.trajectory(a, y0, 1.0 / 64, 64)[-1]
+    Qn = oracle.invariants(oracle.init_explicit(a, tr[None, :], oracle.NULL))[2][0]
+    Qt = oracle.invariants(oracle.init_explicit(a, tr[None, :], oracle.TIMELIKE))[2][0]
+    c2 = (tr[3] / oracle.ks_r(a, *tr[1:4])) ** 2
+    assert abs((Qt - Qn) - a * a * c2) < 1e-12 and c2 > 0.01
+    # u^t re-solved from g u u = -mu^2
+    bad = y0.copy(); bad[4] = 99.0
+    n0 = oracle.invariants(oracle.init_explicit(a, bad[None, :], oracle.NULL, renormalise_ut=True))[3][0]
+    n1 = oracle.invariants(oracle.init_explicit(a, bad[None, :], oracle.TIMELIKE, renormalise_ut=True))[3][0]
+    assert abs(n0) < 1e-13 and abs(n1 + 1.0) < 1e-13
+    assert abs(oracle.init_explicit(a, bad[None, :], oracle.NULL, renormalise_ut=True).q[4, 0] - y0[4]) < 1e-12
+    # init_timelike is the TIMELIKE case
+    t = oracle.init_timelike(a, bad[None, :], renormalise_ut=True)
+    e = oracle.init_explicit(a, bad[None, :], oracle.TIMELIKE, renormalise_ut=True)
+    assert t.kind == oracle.TIMELIKE and np.array_equal(t.q, e.q)
+
+
+def test_clipped_last_step_lands_on_lambda_end_exactly():
+    """DESIGN R22: the clipped step ends at lambda_end itself.  In double 0.03 + (0.283 - 0.03) > 0.283 and
+    0.05 + (0.216 - 0.05) < 0.216, so a clock advanced by lambda += h would overshoot by an ulp in the first
+    case and stop an ulp short -- and take one more, ulp-sized, step -- in the second."""
+    assert 0.03 + (0.283 - 0.03) > 0.283 and 0.05 + (0.216 - 0.05) < 0.216
+    xu8, _ = inputs.cfg1_orbits(4)
+    for driver in (oracle.integrate, oracle.integrate_coordtime):
+        for first, second in ((0.03, 0.283), (0.05, 0.216)):
+            st = oracle.init_timelike(0.0, xu8)
+            sc = oracle.step_control(mode=0, h_fixed=1.0, max_steps=10 ** 6)
+            assert driver(st, first, sc)["steps"] == 4
+            stats = driver(st, second, sc)
+            clock = st.lam if driver is oracle.integrate else st.q[0]
+            assert (clock == second).all() and stats["steps"] == 4 and (st.status == oracle.ACTIVE).all()
+            assert driver(st, second, sc)["steps"] == 0               # a second identical call is a no-op
