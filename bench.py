@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- geodesic RK4 steps/s of the whole hot path on BASELINE.json's headline workload.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype f64|f32] [--workload cfg3|cfg1|cfg2|cfg5]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype both|f64|f32] [--workload cfg3|cfg1|cfg2|cfg5]
     python bench.py --impl reference ...      # the oracle, as it stands, on the host cores
 
 A "step" is one pass of the whole path over one batch: gray2_init_null (image-plane initial conditions)
@@ -11,11 +11,20 @@ the workload north_star quotes the target on.  The metric is geodesic RK4 steps 
 summed over ranks; each rank traces its own image: weak scaling, no collective on the data path;
 --scaling strong shares ONE image among the ranks in tiles of 4096 rays, again without a collective).
 
+BASELINE.json's metric names both precisions, so the default run (--dtype both) times FP64 and then FP32 on
+the same workload: the top-level fields of the JSON line are the FP64 run (BASELINE dtype), the block
+"fp32" carries the same fields for the FP32 run, and "both" the two integrations enqueued together on two
+streams against their serial sum (cfg3 is specified "in both FP64 and FP32").
+
+--gpus N: under torchrun (WORLD_SIZE set) this process is one of the N ranks; without it bench.py starts the
+N ranks itself, one process per GPU, and fails if the box has fewer than N devices.
+
 One JSON line is printed by rank 0; see DESIGN.md "Measurement" for every field.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import math
 import os
@@ -38,12 +47,14 @@ INF = float("inf")
 # (128 FP32 lanes) x 2 flops per FMA x 1.965 GHz (clocks.max.sm of this pool, MEASURED_PEAKS.json).
 FP_LANES = {"f64": 64, "f32": 128}
 
-# DRAM traffic of the dominant kernel, dram__bytes_read.sum + dram__bytes_write.sum per launch, from the
-# `ncu --set full` captures summarised in profiles/r01_ncu_integrate_f{64,32}_v4.txt (cfg3, affine form) and
-# profiles/r01_ncu_integrate_bl_f{64,32}.txt (cfg3, Boyer-Lindquist form).
-# Algorithmic state traffic is 2 x 80 B (FP64) or 2 x 48 B (FP32) per ray.
-NCU_DRAM_BYTES = {("cfg3", "f64", "affine"): 83935744 + 31088896, ("cfg3", "f32", "affine"): 50348544 + 1701632,
-                  ("cfg3", "f64", "bl"): 83937280 + 34206208, ("cfg3", "f32", "bl"): 50350080 + 1716480}
+# Counters of the dominant kernel that only a profiler can give (DRAM bytes per launch from `ncu --set full`,
+# executed FP thread instructions per RK4 step from the ncu op counters / the SASS of the loop) are read from
+# the tracked summary below, keyed by workload, dtype and form; the commands that produced each row are in the
+# .md beside it.  A workload that has no row reports null.
+COUNTERS_CSV = os.path.join(ROOT, "profiles", "kernel_counters.csv")
+
+PROBE_SRC = os.path.join(ROOT, "bench_probe.cu")
+PROBE_LIB = os.path.join(ROOT, "libbench_probe.so")
 
 
 def nominal_peak_tflops(dtype: str, n_sms: int, sm_max_mhz: float) -> float:
@@ -58,10 +69,41 @@ def load_measured_peaks():
         return {}
 
 
+def load_counters(workload: str, dtype: str, form: str):
+    """Row of profiles/kernel_counters.csv for (workload, dtype, form), or None."""
+    try:
+        with open(COUNTERS_CSV) as fh:
+            for row in csv.DictReader(r for r in fh if not r.startswith("#")):
+                if (row["workload"], row["dtype"], row["form"]) == (workload, dtype, form):
+                    return row
+    except Exception:
+        pass
+    return None
+
+
+def build_probe(force: bool = False) -> str:
+    """Compile bench_probe.cu (FMA-only probe kernels; bench-side, not part of libgray2.so) for sm_100a."""
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(PROBE_SRC):
+        tmp = PROBE_LIB + ".tmp.%d" % os.getpid()
+        nvcc = next((c for c in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc") if c and os.path.exists(c)), "nvcc")
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                               "--shared", "-Xcompiler", "-fPIC", "--fmad=false", "-I", ROOT, "-o", tmp, PROBE_SRC])
+        os.replace(tmp, PROBE_LIB)
+    return PROBE_LIB
+
+
+def load_probe():
+    import ctypes as C
+    lib = C.CDLL(build_probe())
+    lib.bench_fma_probe.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+    lib.bench_fma_probe.restype = C.c_int
+    return lib
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks and throttle reasons (profiling recipe).  It is started before the warm-up
     so that nvidia-smi's start-up cost is not inside the timed region; every sample is stamped on arrival
-    and only the samples that fall inside the timed window are reported."""
+    and only the samples that fall inside a timed window are reported."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
@@ -90,13 +132,12 @@ class ClockSampler:
         while self.proc is not None and not self.samples and time.perf_counter() - t0 < timeout:
             time.sleep(0.01)
 
-    def stop(self, t_begin, t_end) -> dict:
+    def window(self, t_begin, t_end) -> dict:
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.05)
-        self.proc.terminate()
         sm, smax, power, reasons = [], [], [], set()
-        for stamp, ln in self.samples:
+        for stamp, ln in list(self.samples):
             if not (t_begin <= stamp <= t_end + 0.03):
                 continue
             parts = [p.strip() for p in ln.split(",")]
@@ -114,6 +155,10 @@ class ClockSampler:
         return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "sm_max_mhz": max(smax),
                 "power_w_max": max(power), "samples": len(sm), "reasons": sorted(reasons)}
 
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
 
 def workload_config(name: str):
     from paper_1706_07062_b200 import inputs
@@ -125,14 +170,10 @@ def workload_config(name: str):
 # reference arm / cpu_baseline: the oracle, as it stands, on the host cores, on a bounded sample
 # ---------------------------------------------------------------------------------------------------
 
-def oracle_sample_config(cfg, side: int):
-    return cfg.scaled(side)
-
-
 def time_oracle(cfg, side: int, steps: int, warmup: int):
     """Each step = init_null + integrate + invariants of the workload's field of view sampled on side^2 rays."""
     import oracle
-    sub = oracle_sample_config(cfg, side)
+    sub = cfg.scaled(side)
     sc = oracle.step_control(mode=1, eta=sub.eta, r_escape=sub.r_escape, max_steps=sub.max_steps,
                              capture_factor=sub.capture_factor)
     total_steps, total_t = 0, 0.0
@@ -172,104 +213,130 @@ def run_reference(args):
 # our arm
 # ---------------------------------------------------------------------------------------------------
 
-def run_gpu(args):
-    import torch
-    import torch.distributed as dist
+class Job:
+    """What every measurement of one rank shares: the workload, the device, the rank layout."""
 
-    from paper_1706_07062_b200 import gray2
+    def __init__(self, args):
+        import torch
+        import torch.distributed as dist
+        from paper_1706_07062_b200 import gray2
+        self.args, self.torch, self.dist, self.gray2 = args, torch, dist, gray2
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+        if self.world != args.gpus:
+            raise SystemExit("bench.py: --gpus %d but WORLD_SIZE = %d" % (args.gpus, self.world))
+        if torch.cuda.device_count() <= self.local:
+            raise SystemExit("bench.py: rank %d needs cuda:%d but the box has %d device(s)"
+                             % (self.rank, self.local, torch.cuda.device_count()))
+        torch.cuda.set_device(self.local)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+        if self.rank == 0:                       # in-tree builds (no-ops when the libraries are up to date)
+            from paper_1706_07062_b200 import build as _build
+            _build.build()
+            build_probe()
+        if self.world > 1:
+            dist.barrier()
+        gray2.load_library()
+        self.probe_lib = load_probe()
+        self.cfg = workload_config(args.workload)
+        self.props = torch.cuda.get_device_properties(self.local)
+        self.n_sms = self.props.multi_processor_count
+        self.sm_max_mhz = float(load_measured_peaks().get("sm_max_mhz", 1965.0))
+        self.coord = args.form == "coordtime"
+        self.bl = args.form == "bl"     # Boyer-Lindquist variant (Table 2 "BL" rows): init -> convert -> integrate
+        cfg = self.cfg
+        self.sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
+                                     capture_factor=cfg.capture_factor)
+        # --scaling strong: ONE image shared by all ranks, rays dealt out in tiles of 4096 (SURVEY 8(e));
+        # weak (default): every rank traces its own image.  Neither has a collective on the data path.
+        self.strong = args.scaling == "strong" and self.world > 1
+        self.n_local = gray2.shard_count(cfg.n, SHARD_TILE, self.rank, self.world) if self.strong else cfg.n
+        self.flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+        try:
+            uuid = str(self.props.uuid)
+            gpu_id = uuid if uuid.startswith("GPU-") else "GPU-" + uuid
+        except Exception:
+            gpu_id = str(self.local)
+        self.sampler = ClockSampler(gpu_id)
+        self.sampler.start()
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if rank == 0:                       # in-tree build (a no-op when libgray2.so is up to date)
-        from paper_1706_07062_b200 import build as _build
-        _build.build()
-    if world > 1:
-        dist.barrier()
-    gray2.load_library()
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
 
-    cfg = workload_config(args.workload)
-    prec = gray2.F64 if args.dtype == "f64" else gray2.F32
-    coord = args.form == "coordtime"
-    bl = args.form == "bl"          # Boyer-Lindquist variant (Table 2 "BL" rows): init -> convert -> integrate
-    flops_per_step = (gray2.flops_per_step_coordtime(prec) if coord else
-                      gray2.flops_per_step_bl(prec) if bl else gray2.flops_per_step(prec))
-    integrate = gray2.integrate_coordtime if coord else gray2.integrate
-    props = torch.cuda.get_device_properties(local)
-    n_sms = props.multi_processor_count
-    peaks = load_measured_peaks()
-    sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    def prec_of(self, dtype):
+        return self.gray2.F64 if dtype == "f64" else self.gray2.F32
+
+    def init_image(self, prec, out=None, stream=None):
+        g, cfg = self.gray2, self.cfg
+        if self.strong:
+            return g.init_null_shard(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, SHARD_TILE,
+                                     self.rank, self.world, prec=prec, out=out, stream=stream)
+        return g.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=out,
+                           stream=stream)
+
+    def flops_per_step(self, prec):
+        g = self.gray2
+        return (g.flops_per_step_coordtime(prec) if self.coord else g.flops_per_step_bl(prec) if self.bl
+                else g.flops_per_step(prec))
+
+    def integrate(self, *a, **kw):
+        return (self.gray2.integrate_coordtime if self.coord else self.gray2.integrate)(*a, **kw)
+
+
+def measure(job: Job, dtype: str) -> dict:
+    """Device-resident timing, end-to-end timing and pipe probes of one precision on this rank.  Returns raw
+    per-rank numbers (times in seconds, work in RK4 steps); run_gpu reduces them over the ranks."""
+    torch, gray2, args, cfg = job.torch, job.gray2, job.args, job.cfg
+    prec = job.prec_of(dtype)
     if args.threads or args.blocks:
         gray2.set_launch(prec, args.threads, args.blocks)
-
-    sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
-                            capture_factor=cfg.capture_factor)
-    # --scaling strong: ONE image shared by all ranks, rays dealt out in tiles of 4096;
-    # weak (default): every rank traces its own image.  Neither has a collective on the data path.
-    strong = args.scaling == "strong" and world > 1
-    n_local = gray2.shard_count(cfg.n, SHARD_TILE, rank, world) if strong else cfg.n
+    n_local, bl = job.n_local, job.bl
     st = gray2.State.empty(n_local, prec)
     st_ks = gray2.State.empty(n_local, prec) if bl else st
     stats = gray2.new_stats()
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     def one_step(ev=None):
         if ev: ev[0].record(stream)
-        if strong:
-            gray2.init_null_shard(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, SHARD_TILE,
-                                  rank, world, prec=prec, out=st_ks)
-        else:
-            gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec, out=st_ks)
+        job.init_image(prec, out=st_ks)
         if bl: gray2.convert(st_ks, gray2.BL, out=st)
         if ev: ev[1].record(stream)
-        integrate(st, INF, sc, stats=stats)
+        job.integrate(st, INF, job.sc, stats=stats)
         if ev: ev[2].record(stream)
         inv = gray2.invariants(st)
         if ev: ev[3].record(stream)
         return inv
 
-    try:
-        gpu_id = "GPU-" + str(props.uuid) if not str(props.uuid).startswith("GPU-") else str(props.uuid)
-    except Exception:
-        gpu_id = str(local)
-    sampler = ClockSampler(gpu_id)
-    sampler.start()
-    for _ in range(max(args.warmup, 3)):
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
         one_step()
     torch.cuda.synchronize()
-    sampler.wait_for_first_sample()
+    job.sampler.wait_for_first_sample()
 
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
+    # ---- device-resident: exactly K steps, L2 flushed before each, CUDA events on the launching stream
+    job.barrier()
     t_window0 = time.perf_counter()
-    t_step, t_int, steps_total = 0.0, 0.0, 0
+    per_step, per_int, steps_total = [], [], 0
     for _ in range(args.steps):
-        flush.fill_(1)                                     # flush L2 between timed iterations (untimed)
+        job.flush.fill_(1)                                     # flush L2 between timed iterations (untimed)
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
         one_step(ev)
         ev[3].synchronize()
-        t_step += ev[0].elapsed_time(ev[3]) * 1e-3
-        t_int += ev[1].elapsed_time(ev[2]) * 1e-3
+        per_step.append(ev[0].elapsed_time(ev[3]) * 1e-3)
+        per_int.append(ev[1].elapsed_time(ev[2]) * 1e-3)
         steps_total += int(stats[0].item())
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    clocks = sampler.stop(t_window0, time.perf_counter())
+    job.barrier()
+    clocks = job.sampler.window(t_window0, time.perf_counter())
 
     # ---- end to end through the public API with HOST buffers (pinned): H2D of the 8-vectors, D2H of results
     host_in = torch.empty((n_local, 8), dtype=torch.float64).pin_memory()
-    if strong:
-        src = gray2.init_null_shard(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, SHARD_TILE,
-                                    rank, world, prec=gray2.F64)
-    else:
-        src = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=gray2.F64)
+    src = job.init_image(gray2.F64)
     host_in.copy_(src.q.t())          # outside the timed region: the user's 8-vectors, resident in host memory
     a_eff = src.a_eff
     del src
@@ -301,15 +368,13 @@ def run_gpu(args):
         for c, (lo, hi) in enumerate(bounds):
             part, ho = parts[c], host_out[c]
             with torch.cuda.stream(streams[c % n_streams]):
+                # explicit null 8-vectors, H2D inside the call
                 if bl:
-                    ks = parts_ks[c]
-                    gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=ks)
-                    ks.kind, ks.reversed = gray2.NULL, 1
-                    gray2.convert(ks, gray2.BL, out=part)
+                    gray2.init_explicit(a_eff, host_in_np[lo:hi], gray2.NULL, prec=prec, out=parts_ks[c])
+                    gray2.convert(parts_ks[c], gray2.BL, out=part)
                 else:
-                    gray2.init_timelike(a_eff, host_in_np[lo:hi], prec=prec, out=part)   # H2D inside (explicit 8-vectors)
-                    part.kind, part.reversed = gray2.NULL, 1
-                integrate(part, INF, sc, stats=chunk_stats[c])
+                    gray2.init_explicit(a_eff, host_in_np[lo:hi], gray2.NULL, prec=prec, out=part)
+                job.integrate(part, INF, job.sc, stats=chunk_stats[c])
                 inv = gray2.invariants(part)
                 ho["q"].copy_(part.q, non_blocking=True); ho["lam"].copy_(part.lam, non_blocking=True)
                 ho["status"].copy_(part.status, non_blocking=True); ho["nsteps"].copy_(part.nsteps, non_blocking=True)
@@ -321,64 +386,173 @@ def run_gpu(args):
 
     e2e_step()
     e2e_n = max(1, min(args.steps, 3))
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
+    job.barrier()
     t0 = time.perf_counter()
     e2e_steps = sum(e2e_step() for _ in range(e2e_n))
     t_e2e = time.perf_counter() - t0
+    del parts, parts_ks, host_out, host_in
 
-    # ---- FMA-only probes of the pipe at the clocks of the moment (context for the nominal peak)
+    # ---- FMA-only probes of the pipe at the clocks of the moment (context for the nominal peak); bench-side kernels
     scratch = torch.zeros(8, dtype=torch.float64 if prec == gray2.F64 else torch.float32, device="cuda")
     iters = 20000 if prec == gray2.F64 else 40000
+    blocks, threads = job.n_sms * 8, 256
     probe = {}
     for name, regs in (("imm", 0), ("regs", 1), ("fresh", 2)) + ((("packed", 3),) if prec == gray2.F32 else ()):
-        gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch, register_operands=regs)
+        def launch():
+            rc = job.probe_lib.bench_fma_probe(int(prec), regs, blocks, threads, iters, scratch.data_ptr(),
+                                               stream.cuda_stream)
+            if rc:
+                raise RuntimeError("bench_fma_probe failed")
+        launch()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        probe_flops = gray2.fma_probe(prec, n_sms * 8, 256, iters, scratch, register_operands=regs)
+        launch()
         e1.record(stream)
         e1.synchronize()
-        probe[name] = probe_flops / (e0.elapsed_time(e1) * 1e-3) / 1e12
-    fma_probe_tflops = probe["imm"]
+        probe[name] = (32 if regs == 3 else 16) * iters * blocks * threads / (e0.elapsed_time(e1) * 1e-3) / 1e12
+    if args.threads or args.blocks:
+        gray2.set_launch(prec, 0, 0)
+    return dict(dtype=dtype, prec=prec, per_step=per_step, per_int=per_int, steps_total=steps_total, clocks=clocks,
+                t_e2e=t_e2e, e2e_steps=e2e_steps, h2d=h2d, d2h=d2h, n_chunks=n_chunks, n_streams=n_streams,
+                probe=probe, warmup=warmup)
 
-    # ---- reduce over ranks: time = max, work = sum
+
+def measure_both(job: Job) -> dict:
+    """cfg3 is specified "in both FP64 and FP32 with identical step rules": the two integrations enqueued together
+    on two streams (launch shapes that fit one SM's register file side by side) against the same two enqueued one
+    after the other.  The FP64 kernel leaves the FP32 pipe idle and the reverse; whether they overlap is measured."""
+    torch, gray2, args = job.torch, job.gray2, job.args
+    s64, s32 = gray2.State.empty(job.n_local, gray2.F64), gray2.State.empty(job.n_local, gray2.F32)
+    st64, st32 = gray2.new_stats(), gray2.new_stats()
+    a, b = torch.cuda.Stream(), torch.cuda.Stream()
+
+    def run(concurrent: bool):
+        job.init_image(gray2.F64, out=s64)
+        job.init_image(gray2.F32, out=s32)
+        job.flush.fill_(1)
+        torch.cuda.synchronize()
+        e0, e1, eb = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(a)
+        b.wait_event(e0)
+        job.integrate(s64, INF, job.sc, stats=st64, stream=a)
+        if not concurrent:
+            mid = torch.cuda.Event()
+            mid.record(a)
+            b.wait_event(mid)
+        job.integrate(s32, INF, job.sc, stats=st32, stream=b)
+        eb.record(b)
+        a.wait_event(eb)
+        e1.record(a)
+        e1.synchronize()
+        return e0.elapsed_time(e1) * 1e-3, int(st64[0].item()) + int(st32[0].item())
+
+    out = {}
+    for name, conc, shapes in (("serial", False, ((0, 0), (0, 0))), ("concurrent", True, ((128, 2), (256, 1)))):
+        gray2.set_launch(gray2.F64, *shapes[0])
+        gray2.set_launch(gray2.F32, *shapes[1])
+        for _ in range(2):
+            run(conc)
+        job.barrier()
+        res = [run(conc) for _ in range(max(3, args.steps))]
+        out[name] = dict(times=[r[0] for r in res], steps=res[0][1])
+    gray2.set_launch(gray2.F64, 0, 0)
+    gray2.set_launch(gray2.F32, 0, 0)
+    return out
+
+
+def block_of(job: Job, m: dict, t_step, t_int, steps_all, t_e2e, e2e_all) -> dict:
+    """The JSON fields of one precision from its reduced numbers (rank 0)."""
+    args, cfg = job.args, job.cfg
+    dtype, prec = m["dtype"], m["prec"]
+    fps = job.flops_per_step(prec)
+    peak = nominal_peak_tflops(dtype, job.n_sms, job.sm_max_mhz)
+    achieved = (m["steps_total"] * fps / sum(m["per_int"])) / 1e12            # this rank's dominant kernel
+    steps_per_pass = m["steps_total"] // args.steps
+    best_int = min(m["per_int"])
+    row = load_counters(args.workload, dtype, args.form) or {}
+    traffic = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"]) if row.get("dram_read_bytes") else None
+    exec_flops = float(row["executed_flops_per_step"]) if row.get("executed_flops_per_step") else None
+    kernel = ("integrate_kernel<double%s>" if dtype == "f64" else "integrate_kernel_f32x2<%s>") % (
+        ", coordinate time" if job.coord else ", Boyer-Lindquist" if job.bl else ("" if dtype == "f64" else "affine"))
+    return {
+        "value": steps_all / t_step, "unit": UNIT, "dtype": dtype,
+        "ms_per_step": 1e3 * t_step / args.steps,
+        "ms_per_step_best": 1e3 * min(m["per_step"]), "ms_per_step_median": 1e3 * statistics.median(m["per_step"]),
+        "value_best": steps_per_pass / min(m["per_step"]) * (job.world if not job.strong else 1),
+        "clocks": m["clocks"],
+        "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"],
+                "api": "gray2_init_explicit(host 8-vectors, NULL) -> %sgray2_integrate -> gray2_invariants -> D2H of state, invariants, stats"
+                       % ("gray2_convert -> " if job.bl else ""),
+                "chunks": m["n_chunks"], "streams": m["n_streams"]},
+        "gpu_launches": (5 if job.bl else 4) * args.steps,
+        "roofline": {"bound": "alu", "kernel": kernel,
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                     "frac_best": steps_per_pass * fps / best_int / 1e12 / peak,
+                     "executed_frac": (m["steps_total"] * exec_flops / sum(m["per_int"]) / 1e12 / peak) if exec_flops else None,
+                     "executed_flops_per_rk4_step": exec_flops,
+                     "executed_source": row.get("executed_source"),
+                     "traffic": traffic,
+                     "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/kernel_counters.csv)",
+                     "algorithmic_bytes": 2 * (80 if dtype == "f64" else 48) * job.n_local,
+                     "flops_per_rk4_step": fps,
+                     "kernel_ms": 1e3 * t_int / args.steps, "kernel_ms_best": 1e3 * best_int,
+                     "kernel_share_of_step": t_int / t_step,
+                     "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (job.n_sms, FP_LANES[dtype], job.sm_max_mhz),
+                     "fma_probe_tflops": m["probe"]["imm"], "frac_of_fma_probe": achieved / m["probe"]["imm"],
+                     "fma_probe_register_operands_tflops": m["probe"]["regs"],
+                     "fma_probe_fresh_register_operands_tflops": m["probe"]["fresh"],
+                     "fma_probe_packed_fp32x2_tflops": m["probe"].get("packed")},
+    }
+
+
+def run_gpu(args):
+    job = Job(args)
+    torch, cfg = job.torch, job.cfg
     from paper_1706_07062_b200 import multi
-    (t_step, t_int, t_e2e), (steps_all, e2e_all) = multi.reduce_job([t_step, t_int, t_e2e], [steps_total, e2e_steps],
-                                                                    device="cuda")
+    dtypes = ["f64", "f32"] if args.dtype == "both" else [args.dtype]
+    blocks = {}
+    for dtype in dtypes:
+        m = measure(job, dtype)
+        # ---- reduce over ranks: time = max, work = sum
+        (t_step, t_int, t_e2e), (steps_all, e2e_all) = multi.reduce_job(
+            [sum(m["per_step"]), sum(m["per_int"]), m["t_e2e"]], [m["steps_total"], m["e2e_steps"]], device="cuda")
+        if job.rank == 0:
+            blocks[dtype] = block_of(job, m, t_step, t_int, steps_all, t_e2e, e2e_all)
+            blocks[dtype]["rk4_steps_per_pass"] = m["steps_total"] // args.steps
+            blocks[dtype]["warmup"] = m["warmup"]
+    both = None
+    if args.dtype == "both" and not job.bl and not job.coord and not args.no_both:
+        b = measure_both(job)
+        (ts, tc), (work,) = multi.reduce_job([statistics.median(b["serial"]["times"]), statistics.median(b["concurrent"]["times"])],
+                                             [b["serial"]["steps"]], device="cuda")
+        both = {"what": "gray2_integrate FP64 and FP32 of the same image: enqueued one after the other (serial) and "
+                        "together on two streams with launch shapes 128x2 (FP64) + 256x1 (FP32) per SM (concurrent)",
+                "ms_serial_sum": 1e3 * ts, "ms_concurrent": 1e3 * tc, "gain": ts / tc,
+                "rk4_steps_both": int(work), "value_concurrent": work / tc, "unit": UNIT}
+    job.sampler.stop()
 
-    if rank == 0:
-        value = steps_all / t_step
-        peak = nominal_peak_tflops(args.dtype, n_sms, sm_max_mhz)
-        achieved = (steps_total * flops_per_step / t_int) / 1e12          # this rank's dominant kernel
+    if job.rank == 0:
+        head = blocks[dtypes[0]]
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * t_step / args.steps, "higher_is_better": True,
-            "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": cfg.name, "rays_per_gpu": n_local, "rk4_steps_per_pass": steps_total // args.steps,
+            "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": job.world, "steps": args.steps,
+            "warmup": head.pop("warmup"), "ms_per_step": head["ms_per_step"], "higher_is_better": True,
+            "scaling": "strong" if job.strong else "weak", "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic",
+            "config": {"workload": cfg.name, "rays_per_gpu": job.n_local, "rk4_steps_per_pass": head.pop("rk4_steps_per_pass"),
                        "a": cfg.a, "r_obs": cfg.r_obs, "inclination_deg": cfg.inclination_deg, "fov_half": cfg.fov,
-                       "form": args.form, "step_rule": ("dt = %g r" if coord else "dlambda = %g r") % cfg.eta, "l2": "flushed between timed iterations (256 MiB fill)",
-                       "parallelism": ("one image dealt out in tiles of %d rays, no collective" % SHARD_TILE) if strong
+                       "form": args.form, "step_rule": ("dt = %g r" if job.coord else "dlambda = %g r") % cfg.eta,
+                       "l2": "flushed between timed iterations (256 MiB fill)",
+                       "parallelism": ("one image dealt out in tiles of %d rays, no collective" % SHARD_TILE) if job.strong
                                       else "independent image per GPU, no collective"},
-            "clocks": clocks,
-            "e2e": {"value": e2e_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "gray2_init_timelike(host 8-vectors) -> %sgray2_integrate -> gray2_invariants -> D2H of state, invariants, stats" % ("gray2_convert -> " if bl else ""),
-                    "chunks": n_chunks, "streams": n_streams},
-            "gpu_launches": (5 if bl else 4) * args.steps,
-            "roofline": {"bound": "alu", "kernel": ("integrate_kernel<double%s>" if prec == gray2.F64 else "integrate_kernel_f32x2<%s>") % (
-                             ", coordinate time" if coord else ", Boyer-Lindquist" if bl else ("" if prec == gray2.F64 else "affine")),
-                         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": NCU_DRAM_BYTES.get((args.workload, args.dtype, args.form)),
-                         "traffic_unit": "bytes per launch (ncu, profiles/r01_ncu_integrate_*.txt)",
-                         "flops_per_rk4_step": flops_per_step,
-                         "kernel_ms": 1e3 * t_int / args.steps, "kernel_share_of_step": t_int / t_step,
-                         "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (n_sms, FP_LANES[args.dtype], sm_max_mhz),
-                         "fma_probe_tflops": fma_probe_tflops, "frac_of_fma_probe": achieved / fma_probe_tflops,
-                         "fma_probe_register_operands_tflops": probe["regs"],
-                         "fma_probe_fresh_register_operands_tflops": probe["fresh"],
-                         "fma_probe_packed_fp32x2_tflops": probe.get("packed")},
         }
-        if not args.no_cpu_baseline and world == 1:
+        for k, v in head.items():
+            line.setdefault(k, v)
+        if len(dtypes) > 1:
+            f32 = blocks["f32"]
+            f32.pop("warmup", None)
+            line["fp32"] = f32
+        if both is not None:
+            line["both"] = both
+        if not args.no_cpu_baseline and job.world == 1:
             # a first pass on oracle_side^2 rays sizes the sample: about 12 s of wall clock on this box's cores
             _, s_probe, _, _ = time_oracle(cfg, args.oracle_side, 1, 0)
             side = int(args.oracle_side * math.sqrt(max(1.0, 12.0 / max(s_probe, 1e-3)))) // 32 * 32
@@ -388,18 +562,46 @@ def run_gpu(args):
                                     "sample": "%s field of view on %dx%d rays, one pass (%.1f s)" % (
                                         args.workload, side, side, s_per)}
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
+    if job.world > 1:
+        job.dist.destroy_process_group()
     return 0
 
 
-def main():
+# ---------------------------------------------------------------------------------------------------
+# --gpus N without torchrun: start the N ranks here, one process per GPU
+# ---------------------------------------------------------------------------------------------------
+
+def _rank_entry(rank: int, world: int, port: int, target, payload):
+    os.environ.update({"RANK": str(rank), "LOCAL_RANK": str(rank), "WORLD_SIZE": str(world),
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    rc = target(payload)
+    if rc:
+        raise SystemExit(rc)
+
+
+def free_port() -> int:
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_ranks(world: int, target, payload) -> int:
+    """Run target(payload) in `world` processes with RANK / LOCAL_RANK / WORLD_SIZE / MASTER_* set as torchrun
+    would (rendezvous on 127.0.0.1).  Raises if a rank fails."""
+    import torch.multiprocessing as mp
+    mp.spawn(_rank_entry, args=(world, free_port(), target, payload), nprocs=world, join=True)
+    return 0
+
+
+def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--dtype", default="both", choices=["both", "f64", "f32"],
+                    help="both (default): FP64 is the headline line, FP32 the block \"fp32\" of the same line")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1 only. weak: one image per GPU; strong: one image shared by the GPUs (tiles of 4096 rays)")
     ap.add_argument("--form", default="affine", choices=["affine", "coordtime", "bl"],
@@ -410,11 +612,24 @@ def main():
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--blocks", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-both", action="store_true", help="skip the two-precisions-at-once leg of --dtype both")
     ap.add_argument("--e2e-chunks", type=int, default=32, help="end-to-end leg: chunks pipelined over the streams")
     ap.add_argument("--e2e-streams", type=int, default=8, help="end-to-end leg: number of streams the chunks alternate between")
-    args = ap.parse_args()
+    args = ap.parse_args(argv)
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: start the ranks here
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit("bench.py: --gpus %d needs %d CUDA devices, this box has %d (the product path has no CPU "
+                             "fallback and ranks do not share a GPU)" % (args.gpus, args.gpus, have))
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # keep the communicator log (nranks) on stderr
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        return launch_ranks(args.gpus, run_gpu, args)
     return run_gpu(args)
 
 

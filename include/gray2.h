@@ -24,14 +24,17 @@
  * library allocates no device memory of its own except a 4 KiB work-queue scratch per device (64 slots
  * handed out round-robin; a call that gets a slot whose previous user is still running waits for it on
  * the device, so any number of integrations may be in flight) and the staging buffers
- * of gray2_init_timelike (n x 64 bytes each, one per calling stream up to eight, grown on demand, reused,
- * released at process exit).  `host_xu8` is a HOST pointer.
+ * of gray2_init_explicit (per device; n x 64 bytes each, one per calling stream up to eight, grown on demand,
+ * reused, released at process exit).  `host_xu8` is a HOST pointer.
  * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
  *
+ * Threads.  Any number of host threads may call into the library at once (the scratch pools are locked, the
+ * launch choice of gray2_set_launch is one atomic word per precision); two calls that write the same
+ * gray2_state must be ordered by the caller.
+ *
  * Devices.  Work runs on the CUDA device that is current in the calling thread; all pointers and the
- * stream must belong to it.  The integrators may be used on several devices of one process (their scratch
- * is per device); gray2_init_timelike keeps its staging buffers on the device of its first call, so a
- * process that feeds explicit 8-vectors to several GPUs needs one process per GPU (the model of bench.py).
+ * stream must belong to it.  Every call may be used on several devices of one process: the library's own
+ * scratch (work queues, staging buffers, copy stream) is kept per device.
  *
  * Asynchrony.  Every call enqueues on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
  * stream) and returns; results are valid after the caller synchronises that stream.
@@ -71,7 +74,7 @@ typedef struct {
   uint64_t n;
   double   a_eff;       /* spin used by the integrator; = -a for states made by gray2_init_null (R3)    */
   int32_t  prec;        /* gray2_precision of q[]                                                       */
-  int32_t  kind;        /* gray2_kind (only gray2_invariants reads it: mu^2 inside Carter's Q)          */
+  int32_t  kind;        /* gray2_kind: mu^2 inside Carter's Q (gray2_invariants) and |u.u + mu^2| (diagnostics) */
   int32_t  reversed;    /* 1: time-reversed ray of a backward trace (physical t = -t, L_z = -L_z)       */
   int32_t  coords;      /* gray2_coords of q[]; set to GRAY2_KS by gray2_init_*, to the target by         */
                         /* gray2_convert; gray2_integrate and gray2_invariants follow it                  */
@@ -117,18 +120,30 @@ int gray2_init_null_shard(gray2_state *s, double a, double r_obs, double inclina
                           uint64_t tile_rays, int32_t rank, int32_t world, void *cuda_stream);
 uint64_t gray2_shard_count(uint64_t n, uint64_t tile_rays, int32_t rank, int32_t world);   /* 0 on bad arguments */
 
-/* Explicit initial conditions.  host_xu8: HOST array of n x 8 doubles (AoS: t,x,y,z,u^t,u^x,u^y,u^z).
- * Copies them into the first n slots of the SoA state (converted to float for F32); with
- * renormalise_ut != 0 replaces u^t by the future-directed root of g u u = -1 (R7).  Sets s->a_eff = a,
- * s->kind = GRAY2_TIMELIKE, s->reversed = 0, lambda = 0, status = ACTIVE, nsteps = 0.  The host array
- * may be reused as soon as the call returns: the call waits for its own host-to-device copy (made on an
- * internal stream, so that it does not queue behind earlier work on cuda_stream) and for nothing else; the
- * state is filled in stream order on cuda_stream like the output of every other call. */
+/* Explicit initial conditions of either kind.  The paper's convergence experiments start from explicit data
+ * for PHOTONS (the six spherical photon orbits of Table 1) and for PARTICLES
+ * (circular orbits with a v_z kick); the state has 8 variables per geodesic.
+ * host_xu8: HOST array of n x 8 doubles (AoS: t,x,y,z,u^t,u^x,u^y,u^z).  Copies them into the first n slots
+ * of the SoA state (converted to float for F32).  kind: GRAY2_NULL (mu^2 = 0) or GRAY2_TIMELIKE (mu^2 = 1);
+ * with renormalise_ut != 0 u^t is replaced by the future-directed root of g u u = -mu^2 (R7).  Sets
+ * s->a_eff = a, s->kind = kind (Carter's Q in gray2_invariants follows it, R8), s->reversed = 0,
+ * lambda = 0, status = ACTIVE, nsteps = 0.  The host array may be reused as soon as the call returns: the
+ * call waits for its own host-to-device copy (made on an internal stream of the current device, so that it
+ * does not queue behind earlier work on cuda_stream) and for nothing else; the state is filled in stream
+ * order on cuda_stream like the output of every other call.  GRAY2_EINVAL for an unknown kind. */
+int gray2_init_explicit(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t kind,
+                        int32_t renormalise_ut, void *cuda_stream);
+/* The call north_star names: gray2_init_explicit with kind = GRAY2_TIMELIKE. */
 int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n,
                         int32_t renormalise_ut, void *cuda_stream);
 
 /* Integrate the first n geodesics of s (see gray2_step_control).  Only ACTIVE geodesics are touched, so
  * the call is resumable and a second identical call is a no-op.  prec must equal s->prec.
+ * FP32 states: the right-hand side is evaluated in float, the eight state sums y <- y + (h/6)(k1+2k2+2k3+k4)
+ * are carried with a float residual each (compensated summation) while a geodesic lives in registers, so
+ * that the low bits of the ~1000 small increments of a ray are not rounded away one by one (DESIGN R12); the
+ * residual is dropped when the geodesic is stored, i.e. at every call boundary the state is plain float.
+ * The clipped last step lands on lambda_end itself (R22).
  * device_stats: DEVICE pointer to one gray2_stats, or NULL; it is OVERWRITTEN with the RK4 steps taken
  * by this call and the final status counts over the first n geodesics.
  *
@@ -213,16 +228,6 @@ int gray2_rhs(int32_t prec, double a, uint64_t n, const void *pos, const void *u
 /* The same for the Boyer-Lindquist right-hand side: pos (2 n: r.., theta..), u (4 n: u^t.., u^r.., u^theta..,
  * u^phi..), out (4 n). */
 int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void *u, void *out, void *cuda_stream);
-
-/* Diagnostic entry: FMA-only probe kernel (8 independent chains per thread) for measuring the attainable
- * FMA rate of the FP64 / FP32 pipe.  register_operands = 0: multiplier and addend are immediates (best
- * case of the pipe); 1: three per-thread register operands, multiplier and addend shared by the chains;
- * 2: every chain has its own multiplier and addend, three fresh register reads per FMA (what real code
- * issues; bounded by register-file read bandwidth); 3 (GRAY2_F32 only): as 2, made of the packed FFMA2
- * instruction of the default FP32 integrator.  scratch: DEVICE pointer, >= 1 element.
- * Flops = 16*iters*blocks*threads (32*iters*blocks*threads for the packed probe). */
-int gray2_fma_probe(int32_t prec, int32_t register_operands, int32_t blocks, int32_t threads, int32_t iters,
-                    void *scratch, void *cuda_stream);
 
 const char *gray2_last_error(void);   /* thread-local text of the last error of the calling thread */
 const char *gray2_version(void);

@@ -133,11 +133,11 @@ template <> __device__ __forceinline__ double min_<double>(double a, double b) {
 template <> __device__ __forceinline__ float min_<float>(float a, float b) { return fminf(a, b); }
 
 // Classic RK4; Ray<T> holds (t, r, theta, phi, t', r', theta', phi') in (t, x, y, z, u0..u3).
-// The result goes to `o`; the return value is the smallest radius among the positions of stages 2-4 and the
+// The result goes to `o` (and the residuals of the FP32 sums to `oc`); the return value is the smallest radius among the positions of stages 2-4 and the
 // result.  Eq. (1) is singular at Delta = 0 and a stage evaluated at or beyond the horizon is meaningless, so
 // the caller accepts the step only if that radius is still outside the capture radius (DESIGN R20).
 template <typename T, typename K>
-__device__ __forceinline__ T rk4_step_bl(const SpinConst<T> &k, const Ray<T> &s, T h, Ray<T> &o) {
+__device__ __forceinline__ T rk4_step_bl(const SpinConst<T> &k, const Ray<T> &s, const Carry<T> &c, T h, Ray<T> &o, Carry<T> &oc) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
   T b0, b1, b2, b3, v0, v1, v2, v3, pr, pth, rmin;
   T St, Sr, Sth, Sph, S0, S1, S2, S3;
@@ -164,14 +164,16 @@ __device__ __forceinline__ T rk4_step_bl(const SpinConst<T> &k, const Ray<T> &s,
   rmin = min_(rmin, pr);
   // stage 4
   bl_accel<T, K>(k, pr, pth, v0, v1, v2, v3, b0, b1, b2, b3);
-  o.t = fma_(h6, St + v0, s.t);
-  o.x = fma_(h6, Sr + v1, s.x);
-  o.y = fma_(h6, Sth + v2, s.y);
-  o.z = fma_(h6, Sph + v3, s.z);
-  o.u0 = fma_(h6, S0 + b0, s.u0);
-  o.u1 = fma_(h6, S1 + b1, s.u1);
-  o.u2 = fma_(h6, S2 + b2, s.u2);
-  o.u3 = fma_(h6, S3 + b3, s.u3);
+  o = s;
+  oc = c;
+  if constexpr (!Carry<T>::compensated) {      // double: plain sums
+    advance(o.t, h6, St + v0); advance(o.x, h6, Sr + v1); advance(o.y, h6, Sth + v2); advance(o.z, h6, Sph + v3);
+    advance(o.u0, h6, S0 + b0); advance(o.u1, h6, S1 + b1); advance(o.u2, h6, S2 + b2); advance(o.u3, h6, S3 + b3);
+  } else {                                                 // FP32: compensated sums (Carry, ks_geodesic.cuh)
+    advance(o.t, oc.t, h6, St + v0); advance(o.x, oc.x, h6, Sr + v1); advance(o.y, oc.y, h6, Sth + v2);
+    advance(o.z, oc.z, h6, Sph + v3); advance(o.u0, oc.u0, h6, S0 + b0); advance(o.u1, oc.u1, h6, S1 + b1);
+    advance(o.u2, oc.u2, h6, S2 + b2); advance(o.u3, oc.u3, h6, S3 + b3);
+  }
   return min_(rmin, o.x);
 }
 

@@ -54,11 +54,15 @@ template <int C> __device__ __forceinline__ void set_half(f32x2 &a, float s) {
   if (C == 0) a.v.x = s; else a.v.y = s;
 }
 
-// copy half C of every variable of a packed ray
-template <int C> __device__ __forceinline__ void copy_half(Ray<f32x2> &d, const Ray<f32x2> &s) {
+// copy half C of every variable of a packed ray (or of its residuals)
+template <int C, typename R> __device__ __forceinline__ void copy_half(R &d, const R &s) {
   set_half<C>(d.t, half_of<C>(s.t)); set_half<C>(d.x, half_of<C>(s.x)); set_half<C>(d.y, half_of<C>(s.y));
   set_half<C>(d.z, half_of<C>(s.z)); set_half<C>(d.u0, half_of<C>(s.u0)); set_half<C>(d.u1, half_of<C>(s.u1));
   set_half<C>(d.u2, half_of<C>(s.u2)); set_half<C>(d.u3, half_of<C>(s.u3));
+}
+template <int C> __device__ __forceinline__ void clear_half(Carry<f32x2> &c) {
+  set_half<C>(c.t, 0.0f); set_half<C>(c.x, 0.0f); set_half<C>(c.y, 0.0f); set_half<C>(c.z, 0.0f);
+  set_half<C>(c.u0, 0.0f); set_half<C>(c.u1, 0.0f); set_half<C>(c.u2, 0.0f); set_half<C>(c.u3, 0.0f);
 }
 
 }  // namespace gray2

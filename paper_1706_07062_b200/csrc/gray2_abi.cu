@@ -7,6 +7,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
 #include <mutex>
 
 #include "../../include/gray2.h"
@@ -79,9 +80,17 @@ int acquire_slot(cudaStream_t st, QueueSlot *out) {
   return GRAY2_OK;
 }
 
+// ---- staging buffers of gray2_init_explicit: per device, one slot per calling stream -----------------
+constexpr int kStages = 8;
+struct Stage { cudaStream_t key; bool made; double *buf; size_t bytes; cudaEvent_t copied, consumed; };
+struct StagePool { Stage slot[kStages] = {}; cudaStream_t copy_stream = nullptr; unsigned next = 0; };
+StagePool g_stages[kMaxDevices];
+std::mutex g_stage_lock;
+
 // ---- launch configuration of the integrator (gray2_set_launch) ------------------------------------
-int g_threads[2] = {0, 0};          // 0 = default
-int g_blocks_per_sm[2] = {0, 0};
+// (threads << 16) | blocks_per_sm in ONE atomic word per precision, 0 = default, so that an integration that
+// races with gray2_set_launch sees either the old pair or the new one, never a mixture.
+std::atomic<uint32_t> g_launch[2] = {{0u}, {0u}};
 
 template <typename T> gray2::StateView<T> view_of(const gray2_state *s) {
   gray2::StateView<T> v;
@@ -144,12 +153,13 @@ cudaError_t launch_integrate_x2(const gray2_state *s, uint64_t n, const gray2::S
 struct LaunchChoice { int threads, blocks; };
 
 // Compiled variants of the affine-parameter integrator; the first entry of each list is the default
-// and the only one compiled for the coordinate-time form and for the Boyer-Lindquist form.  FP32: the first three entries run two
-// geodesics per thread (integrate_kernel_f32x2), the last two one per thread (integrate_kernel<float>);
-// every variant gives bit-identical results.
-constexpr int kNumVariants = 5;
-constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}, {256, 1}, {128, 2}};
-constexpr LaunchChoice kF32Variants[kNumVariants] = {{256, 2}, {128, 3}, {128, 4}, {128, 8}, {128, 6}};
+// and the only one compiled for the coordinate-time form and for the Boyer-Lindquist form.  FP32: the entries
+// 256x2, 128x3, 128x4 and 256x1 run two geodesics per thread (integrate_kernel_f32x2), 128x8 and 128x6 one per
+// thread (integrate_kernel<float>); every variant gives bit-identical results.  FP64 128x2 + FP32 256x1 are the
+// pair that fits one SM's register file side by side (both precisions of one image at once, bench.py "both").
+constexpr int kNumVariants = 6;
+constexpr LaunchChoice kF64Variants[kNumVariants] = {{128, 3}, {128, 4}, {64, 6}, {256, 1}, {128, 2}, {128, 1}};
+constexpr LaunchChoice kF32Variants[kNumVariants] = {{256, 2}, {128, 3}, {128, 4}, {128, 8}, {128, 6}, {256, 1}};
 
 template <typename T>
 cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_state *s, uint64_t n,
@@ -166,6 +176,7 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, sms, st);
     GRAY2_VARIANT(128, 3) GRAY2_VARIANT(128, 4) GRAY2_VARIANT(64, 6) GRAY2_VARIANT(256, 1) GRAY2_VARIANT(128, 2)
+    GRAY2_VARIANT(128, 1)
 #undef GRAY2_VARIANT
   } else {
     if (form == 1) return launch_integrate_x2<256, 2, 1>(s, n, p, q, steps, sms, st);
@@ -178,7 +189,7 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
   if (threads == TH && blocks == BL) return launch_integrate_x2<TH, BL, 0>(s, n, p, q, steps, sms, st);
 #define GRAY2_VARIANT(TH, BL) \
   if (threads == TH && blocks == BL) return launch_integrate<T, TH, BL, 0>(s, n, p, q, steps, sms, st);
-    GRAY2_VARIANT_X2(128, 4) GRAY2_VARIANT_X2(128, 3) GRAY2_VARIANT_X2(256, 2)
+    GRAY2_VARIANT_X2(128, 4) GRAY2_VARIANT_X2(128, 3) GRAY2_VARIANT_X2(256, 2) GRAY2_VARIANT_X2(256, 1)
     GRAY2_VARIANT(128, 8) GRAY2_VARIANT(128, 6)
 #undef GRAY2_VARIANT
 #undef GRAY2_VARIANT_X2
@@ -220,8 +231,9 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double end, const gray2
 
   const int pi = sizeof(T) == 8 ? 0 : 1;
   const LaunchChoice def = sizeof(T) == 8 ? kF64Variants[0] : kF32Variants[0];
-  int threads = g_threads[pi] ? g_threads[pi] : def.threads;
-  int blocks = g_blocks_per_sm[pi] ? g_blocks_per_sm[pi] : def.blocks;
+  const uint32_t chosen = g_launch[pi].load(std::memory_order_relaxed);
+  int threads = chosen ? (int)(chosen >> 16) : def.threads;
+  int blocks = chosen ? (int)(chosen & 0xffffu) : def.blocks;
   bool found = false;
   cudaError_t e = dispatch_integrate<T>(form, threads, blocks, s, n, p, queue, steps, qs.num_sms, st, &found);
   if (!found) return fail(GRAY2_EINVAL, "gray2_integrate: no compiled variant for %d threads x %d blocks/SM", threads, blocks);
@@ -277,7 +289,7 @@ int diag_impl(gray2_state *s, uint64_t n, double lambda_end, const gray2_step_co
 extern "C" {
 
 const char *gray2_last_error(void) { return g_err; }
-const char *gray2_version(void) { return "gray2-b200 0.1 (sm_100a)"; }
+const char *gray2_version(void) { return "gray2-b200 0.2 (sm_100a)"; }
 
 /* Number of rays of rank `rank` when n rays are dealt out in tiles of tile_rays, tile t to rank t mod world. */
 uint64_t gray2_shard_count(uint64_t n, uint64_t tile_rays, int32_t rank, int32_t world) {
@@ -325,38 +337,40 @@ int gray2_init_null(gray2_state *s, double a, double r_obs, double inc, double W
   return gray2_init_null_shard(s, a, r_obs, inc, Wa, Wb, nx, ny, (uint64_t)nx * (uint64_t)ny, 0, 1, cuda_stream);
 }
 
-int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t renorm,
+int gray2_init_explicit(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t kind, int32_t renorm,
                         void *cuda_stream) {
+  const char *who = "gray2_init_explicit";
   if (s) s->coords = GRAY2_KS;
-  int rc = check_state(s, "gray2_init_timelike");
+  int rc = check_state(s, who);
   if (rc) return rc;
-  if (!host_xu8 || n == 0) return fail(GRAY2_EINVAL, "gray2_init_timelike: host_xu8 is NULL or n == 0");
-  if (n > s->n) return fail(GRAY2_ESTATE, "gray2_init_timelike: n (%llu) exceeds s->n (%llu)", (unsigned long long)n, (unsigned long long)s->n);
-  if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "gray2_init_timelike: |a| must be <= 1 (got %g)", a);
+  if (!host_xu8 || n == 0) return fail(GRAY2_EINVAL, "%s: host_xu8 is NULL or n == 0", who);
+  if (n > s->n) return fail(GRAY2_ESTATE, "%s: n (%llu) exceeds s->n (%llu)", who, (unsigned long long)n, (unsigned long long)s->n);
+  if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a| must be <= 1 (got %g)", who, a);
+  if (kind != GRAY2_NULL && kind != GRAY2_TIMELIKE) return fail(GRAY2_EINVAL, "%s: kind must be GRAY2_NULL or GRAY2_TIMELIKE", who);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  // Staging buffers for the AoS input: owned by the library, grown on demand and reused (a fresh
-  // stream-ordered allocation per call costs up to 100 ms when the pool has to grow again).  A small pool,
-  // one slot per calling stream (round robin beyond kStages streams).  The host-to-device copy runs on an
-  // internal stream, so that it does not queue behind the caller's earlier work on `st` (a caller that
-  // pipelines chunks over a few streams gets its inputs prefetched while earlier chunks integrate); the
-  // caller's stream waits for the copy, the next copy into a slot waits for the kernel that consumed it, and
-  // the host waits only for its own copy, after which host_xu8 may be reused.
-  constexpr int kStages = 8;
-  struct Stage { cudaStream_t key; bool made; double *buf; size_t bytes; cudaEvent_t copied, consumed; };
-  static std::mutex stage_lock;
-  static Stage stages[kStages] = {};
-  static cudaStream_t copy_stream = nullptr;
-  static unsigned next_slot = 0;
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return fail(GRAY2_ECUDA, "device ordinal %d out of range", dev);
+  // Staging buffers for the AoS input: owned by the library, per device (like the work-queue scratch), grown
+  // on demand and reused (a fresh stream-ordered allocation per call costs up to 100 ms when the pool has to
+  // grow again).  A small pool, one slot per calling stream (round robin beyond kStages streams).  The
+  // host-to-device copy runs on an internal stream of that device, so that it does not queue behind the
+  // caller's earlier work on `st` (a caller that pipelines chunks over a few streams gets its inputs
+  // prefetched while earlier chunks integrate); the caller's stream waits for the copy, the next copy into a
+  // slot waits for the kernel that consumed it, and the host waits only for its own copy, after which
+  // host_xu8 may be reused.
   const size_t bytes = (size_t)n * 8 * sizeof(double);
+  const double mu2 = kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
   cudaEvent_t copied;
   {
-    std::lock_guard<std::mutex> guard(stage_lock);
-    if (!copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+    std::lock_guard<std::mutex> guard(g_stage_lock);
+    StagePool &pool = g_stages[dev];
+    if (!pool.copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&pool.copy_stream, cudaStreamNonBlocking));
     Stage *sl = nullptr;
     for (int i = 0; i < kStages && !sl; ++i)
-      if (stages[i].made && stages[i].key == st) sl = &stages[i];
+      if (pool.slot[i].made && pool.slot[i].key == st) sl = &pool.slot[i];
     if (!sl) {
-      sl = &stages[next_slot++ % kStages];
+      sl = &pool.slot[pool.next++ % kStages];
       if (!sl->made) {
         CUDA_TRY(cudaEventCreateWithFlags(&sl->copied, cudaEventDisableTiming));
         CUDA_TRY(cudaEventCreateWithFlags(&sl->consumed, cudaEventDisableTiming));
@@ -369,22 +383,27 @@ int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64
       CUDA_TRY(cudaMalloc(&sl->buf, bytes));
       sl->bytes = bytes;
     }
-    CUDA_TRY(cudaStreamWaitEvent(copy_stream, sl->consumed, 0));      // the kernel that last read this slot
-    CUDA_TRY(cudaMemcpyAsync(sl->buf, host_xu8, bytes, cudaMemcpyHostToDevice, copy_stream));
-    CUDA_TRY(cudaEventRecord(sl->copied, copy_stream));
+    CUDA_TRY(cudaStreamWaitEvent(pool.copy_stream, sl->consumed, 0));      // the kernel that last read this slot
+    CUDA_TRY(cudaMemcpyAsync(sl->buf, host_xu8, bytes, cudaMemcpyHostToDevice, pool.copy_stream));
+    CUDA_TRY(cudaEventRecord(sl->copied, pool.copy_stream));
     CUDA_TRY(cudaStreamWaitEvent(st, sl->copied, 0));
     unsigned grid = (unsigned)((n + 255) / 256);
     if (s->prec == GRAY2_F64)
-      gray2::init_explicit_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), sl->buf, n, a, renorm);
+      gray2::init_explicit_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), sl->buf, n, a, renorm, mu2);
     else
-      gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), sl->buf, n, a, renorm);
+      gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), sl->buf, n, a, renorm, mu2);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaEventRecord(sl->consumed, st));
     copied = sl->copied;
   }
   CUDA_TRY(cudaEventSynchronize(copied));   // host_xu8 may be reused on return
-  s->a_eff = a; s->kind = GRAY2_TIMELIKE; s->reversed = 0; s->coords = GRAY2_KS;
+  s->a_eff = a; s->kind = kind; s->reversed = 0; s->coords = GRAY2_KS;
   return GRAY2_OK;
+}
+
+int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t renorm,
+                        void *cuda_stream) {
+  return gray2_init_explicit(s, a, host_xu8, n, GRAY2_TIMELIKE, renorm, cuda_stream);
 }
 
 // Arguments common to gray2_integrate, gray2_integrate_coordtime and gray2_integrate_diagnostics.
@@ -550,45 +569,13 @@ int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 534; }
  *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 598 / 566 per step. */
 int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 566 : 598; }
 
-/* Diagnostic entry: enqueue an FMA-only kernel (blocks x threads threads, 8*iters FMAs each) so that the
- * caller can time the attainable FMA rate of the FP64 / FP32 pipe at the clocks of the moment.
- * register_operands = 0: multiplier and addend are immediates; 1: three per-thread register operands, two of
- * them shared by the chains; 2: three register operands per FMA, none shared with the neighbouring FMAs;
- * 3 (GRAY2_F32 only): as 2 with the packed FFMA2 instruction, two floats per operand, flops = 32*iters*blocks*threads.
- * scratch: DEVICE pointer to at least one element of the precision's type.  Flops = 16*iters*blocks*threads. */
-int gray2_fma_probe(int32_t prec, int32_t register_operands, int32_t blocks, int32_t threads, int32_t iters,
-                    void *scratch, void *cuda_stream) {
-  if (!scratch || blocks <= 0 || threads <= 0 || threads > 1024 || iters <= 0)
-    return fail(GRAY2_EINVAL, "gray2_fma_probe: bad argument");
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  if (register_operands == 3) {
-    if (prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_fma_probe: the packed probe (3) exists for GRAY2_F32 only");
-    gray2::fma2_probe_kernel<<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
-    CUDA_TRY(cudaGetLastError());
-    return GRAY2_OK;
-  }
-  if (register_operands < 0 || register_operands > 3) return fail(GRAY2_EINVAL, "gray2_fma_probe: register_operands must be 0, 1, 2 or 3");
-  if (prec == GRAY2_F64) {
-    if (register_operands == 2) gray2::fma_probe_kernel<double, 2><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
-    else if (register_operands) gray2::fma_probe_kernel<double, 1><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
-    else gray2::fma_probe_kernel<double, 0><<<blocks, threads, 0, st>>>(iters, 1.0, (double *)scratch);
-  } else if (prec == GRAY2_F32) {
-    if (register_operands == 2) gray2::fma_probe_kernel<float, 2><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
-    else if (register_operands) gray2::fma_probe_kernel<float, 1><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
-    else gray2::fma_probe_kernel<float, 0><<<blocks, threads, 0, st>>>(iters, 1.0f, (float *)scratch);
-  } else return fail(GRAY2_EINVAL, "gray2_fma_probe: unknown precision");
-  CUDA_TRY(cudaGetLastError());
-  return GRAY2_OK;
-}
-
 int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm) {
   if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_set_launch: unknown precision");
   const LaunchChoice *list = prec == GRAY2_F64 ? kF64Variants : kF32Variants;
   bool ok = threads_per_block == 0 && blocks_per_sm == 0;
   for (int i = 0; i < kNumVariants && !ok; ++i) ok = list[i].threads == threads_per_block && list[i].blocks == blocks_per_sm;
   if (!ok) return fail(GRAY2_EINVAL, "gray2_set_launch: %d x %d is not a compiled variant", threads_per_block, blocks_per_sm);
-  g_threads[prec] = threads_per_block;
-  g_blocks_per_sm[prec] = blocks_per_sm;
+  g_launch[prec].store(((uint32_t)threads_per_block << 16) | (uint32_t)blocks_per_sm, std::memory_order_relaxed);
   return GRAY2_OK;
 }
 

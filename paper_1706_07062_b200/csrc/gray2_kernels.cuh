@@ -78,13 +78,13 @@ __global__ void init_null_kernel(StateView<T> s, uint64_t n_local, double a_eff,
 
 template <typename T>
 __global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ xu8, uint64_t n, double a,
-                                     int32_t renorm) {
+                                     int32_t renorm, double mu2) {
   uint64_t idx = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= n) return;
   const double2 *row = reinterpret_cast<const double2 *>(xu8 + idx * 8);
   double2 v0 = row[0], v1 = row[1], v2 = row[2], v3 = row[3];
   double ut = v2.x;
-  if (renorm) ut = solve_ut(a, v0.y, v1.x, v1.y, v2.y, v3.x, v3.y, 1.0);
+  if (renorm) ut = solve_ut(a, v0.y, v1.x, v1.y, v2.y, v3.x, v3.y, mu2);
   s.q[0][idx] = T(v0.x); s.q[1][idx] = T(v0.y); s.q[2][idx] = T(v1.x); s.q[3][idx] = T(v1.y);
   s.q[4][idx] = T(ut); s.q[5][idx] = T(v2.y); s.q[6][idx] = T(v3.x); s.q[7][idx] = T(v3.y);
   s.lambda[idx] = 0.0; s.status[idx] = GRAY2_ACTIVE; s.nsteps[idx] = 0;
@@ -115,6 +115,8 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
   ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = T(0);
   ray.z = T(3);                // idle lanes integrate a harmless dummy state (never stored)
   if constexpr (FORM == 2) { ray.x = T(3); ray.y = T(1); }
+  Carry<T> car;                // FP32: residuals of the compensated state sums (empty in double)
+  car.clear();
   double lam = 0.0;
   int32_t nst = 0, nst0 = 0;
   uint64_t idx = 0;
@@ -147,6 +149,7 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
             lam = s.lambda[idx];
           }
           nst = nst0 = s.nsteps[idx];
+          car.clear();
           have = true;
         }
       }
@@ -192,22 +195,24 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
         break;
       }
       T h = (MODE == 1) ? p.eta_or_h * g.r : p.eta_or_h;
-      double hd = (double)h;
+      double lam_next = lam + (double)h;
       if (CLIP) {
+        // the clipped last step lands on lambda_end itself (DESIGN R22)
         double rem = p.lambda_end - lam;
-        if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
+        if (fabs((double)h) > fabs(rem)) { h = (T)rem; lam_next = p.lambda_end; }
       }
       if constexpr (FORM == 2) {
         // the step is accepted only if no stage position, and not its result, is inside the capture radius;
         // otherwise the geodesic ends as CAPTURED at the state it has now (DESIGN R20)
         Ray<T> nxt;
-        T rmin = rk4_step_bl<T, TrigConst<T>>(k, ray, h, nxt);
+        Carry<T> ncar;
+        T rmin = rk4_step_bl<T, TrigConst<T>>(k, ray, car, h, nxt, ncar);
         if (rmin < p.r_capture) cap = true;
-        else { ray = nxt; lam += hd; nst += 1; }
+        else { ray = nxt; car = ncar; lam = lam_next; nst += 1; }
       } else {
-        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, w, h);
-        else rk4_step(k, ray, g, w, h);
-        lam += hd;
+        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, car, g, w, h);
+        else rk4_step(k, ray, car, g, w, h);
+        lam = lam_next;
         nst += 1;
       }
     }
@@ -231,7 +236,7 @@ struct PairSlot {
 
 template <int C, int FORM>
 __device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, uint64_t mine, Ray<f32x2> &ray,
-                                          PairSlot &sl) {
+                                          Carry<f32x2> &car, PairSlot &sl) {
   if (mine < n && s.status[mine] == GRAY2_ACTIVE) {
     sl.idx = mine;
     float t = s.q[0][mine], u0 = s.q[4][mine], u1 = s.q[5][mine], u2 = s.q[6][mine], u3 = s.q[7][mine];
@@ -246,6 +251,7 @@ __device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n,
     set_half<C>(ray.z, s.q[3][mine]); set_half<C>(ray.u0, u0); set_half<C>(ray.u1, u1);
     set_half<C>(ray.u2, u2); set_half<C>(ray.u3, u3);
     sl.nst = sl.nst0 = s.nsteps[mine];
+    clear_half<C>(car);
     sl.have = true;
     sl.cap = false;
   }
@@ -294,6 +300,8 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
   ray.t = ray.x = ray.y = ray.u0 = ray.u1 = ray.u2 = ray.u3 = f32x2(0.0f);
   ray.z = f32x2(3.0f);         // idle slots integrate a harmless dummy state (never stored)
   if constexpr (FORM == 2) { ray.x = f32x2(3.0f); ray.y = f32x2(1.0f); }
+  Carry<f32x2> car;            // residuals of the compensated state sums (ks_geodesic.cuh)
+  car.clear();
   PairSlot A{0, 0.0, 0, 0, false, false}, B{0, 0.0, 0, 0, false, false};
   bool drained = false;
   unsigned long long my_steps = 0;
@@ -306,8 +314,8 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
       if (lane == 0) base = atomicAdd(queue, (unsigned long long)cnt);
       base = __shfl_sync(0xffffffffu, base, 0);
       if (base + cnt >= n) drained = true;
-      if (!A.have) load_slot<0, FORM>(s, n, base + __popc(idleA & lt_mask), ray, A);
-      if (!B.have) load_slot<1, FORM>(s, n, base + cntA + __popc(idleB & lt_mask), ray, B);
+      if (!A.have) load_slot<0, FORM>(s, n, base + __popc(idleA & lt_mask), ray, car, A);
+      if (!B.have) load_slot<1, FORM>(s, n, base + cntA + __popc(idleB & lt_mask), ray, car, B);
       continue;
     }
     if ((idleA & idleB) == 0xffffffffu) break;
@@ -332,23 +340,25 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
         break;
       }
       f32x2 h = (MODE == 1) ? f32x2(p.eta_or_h) * g.r : f32x2(p.eta_or_h);
-      double hdA = (double)h.v.x, hdB = (double)h.v.y;
+      double nextA = A.lam + (double)h.v.x, nextB = B.lam + (double)h.v.y;
       if (CLIP) {
+        // the clipped last step lands on lambda_end itself (DESIGN R22)
         double remA = p.lambda_end - A.lam, remB = p.lambda_end - B.lam;
-        if (fabs(hdA) > fabs(remA)) { hdA = remA; h.v.x = (float)remA; }
-        if (fabs(hdB) > fabs(remB)) { hdB = remB; h.v.y = (float)remB; }
+        if (fabs((double)h.v.x) > fabs(remA)) { h.v.x = (float)remA; nextA = p.lambda_end; }
+        if (fabs((double)h.v.y) > fabs(remB)) { h.v.y = (float)remB; nextB = p.lambda_end; }
       }
       if constexpr (FORM == 2) {
         Ray<f32x2> nxt;
-        f32x2 rmin = rk4_step_bl<f32x2, TrigConst<float>>(k, ray, h, nxt);
+        Carry<f32x2> ncar;
+        f32x2 rmin = rk4_step_bl<f32x2, TrigConst<float>>(k, ray, car, h, nxt, ncar);
         if (rmin.v.x < p.r_capture) A.cap = true;
-        else { copy_half<0>(ray, nxt); A.lam += hdA; A.nst += 1; }
+        else { copy_half<0>(ray, nxt); copy_half<0>(car, ncar); A.lam = nextA; A.nst += 1; }
         if (rmin.v.y < p.r_capture) B.cap = true;
-        else { copy_half<1>(ray, nxt); B.lam += hdB; B.nst += 1; }
+        else { copy_half<1>(ray, nxt); copy_half<1>(car, ncar); B.lam = nextB; B.nst += 1; }
       } else {
-        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, g, w, h);
-        else rk4_step(k, ray, g, w, h);
-        A.lam += hdA; B.lam += hdB;
+        if constexpr (FORM == 1) rk4_step_coordtime(k, ray, car, g, w, h);
+        else rk4_step(k, ray, car, g, w, h);
+        A.lam = nextA; B.lam = nextB;
         A.nst += 1; B.nst += 1;
       }
     }
@@ -387,6 +397,8 @@ __global__ void integrate_diag_kernel(StateView<T> s, uint64_t n, StepParams<T> 
   Ray<T> ray;
   ray.t = s.q[0][idx]; ray.x = s.q[1][idx]; ray.y = s.q[2][idx]; ray.z = s.q[3][idx];
   ray.u0 = s.q[4][idx]; ray.u1 = s.q[5][idx]; ray.u2 = s.q[6][idx]; ray.u3 = s.q[7][idx];
+  Carry<T> car;
+  car.clear();
   double lam = s.lambda[idx];
   int32_t nst = s.nsteps[idx], nst0 = nst, st = GRAY2_ACTIVE;
   // accumulators
@@ -416,7 +428,7 @@ __global__ void integrate_diag_kernel(StateView<T> s, uint64_t n, StepParams<T> 
           peak = c1 - (c - c2) * (c - c2) / (8.0 * (c2 - 2.0 * c1 + c));
           have_peak = true;
         }
-        if (!have_dphi && ks >= 2 && zprev < 0.0 && z >= 0.0) {
+        if (!have_dphi && zprev < 0.0 && z >= 0.0) {         // ks >= 1 here: the pair (z_0, z_1) counts
           double w = -zprev / (z - zprev);
           dphi = phiunf + w * (unf - phiunf) - phi0;
           have_dphi = true;
@@ -436,10 +448,10 @@ __global__ void integrate_diag_kernel(StateView<T> s, uint64_t n, StepParams<T> 
     if (nst >= p.max_steps) { st = GRAY2_MAXSTEPS; break; }
     if (p.dir * (p.lambda_end - lam) <= 0.0) break;
     T h = (MODE == 1) ? p.eta_or_h * g.r : p.eta_or_h;
-    double hd = (double)h, rem = p.lambda_end - lam;
-    if (fabs(hd) > fabs(rem)) { hd = rem; h = (T)rem; }
-    rk4_step(k, ray, g, w, h);
-    lam += hd;
+    double lam_next = lam + (double)h, rem = p.lambda_end - lam;
+    if (fabs((double)h) > fabs(rem)) { h = (T)rem; lam_next = p.lambda_end; }     // DESIGN R22
+    rk4_step(k, ray, car, g, w, h);
+    lam = lam_next;
     nst += 1;
   }
   s.q[0][idx] = ray.t; s.q[1][idx] = ray.x; s.q[2][idx] = ray.y; s.q[3][idx] = ray.z;
@@ -588,63 +600,6 @@ __global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos
   T a0, a1, a2, a3;
   ks_accel(k, g, pos[i], pos[n + i], u[i], u[n + i], u[2 * n + i], u[3 * n + i], a0, a1, a2, a3);
   out[i] = a0; out[n + i] = a1; out[2 * n + i] = a2; out[3 * n + i] = a3;
-}
-
-// Diagnostic: FMA-only probe of the FP64 / FP32 pipe (8 independent chains per thread, registers only).
-// Each thread executes 8 * iters FMAs; the launch's flop count is 2 * 8 * iters * threads.
-// REGS = 0: multiplier and addend are immediates (the pipe's best case);
-// REGS = 1: all three operands are registers that differ per thread, multiplier and addend shared by the
-//           eight chains (consecutive instructions find two of their operands in the operand-reuse cache);
-// REGS = 2: every chain has its own multiplier and addend, so that no instruction shares a source register
-//           with its neighbours -- three fresh register reads per FMA, the mix real code issues, which on
-//           B200 is limited by register-file read bandwidth rather than by the pipe.
-template <typename T, int REGS>
-__global__ void fma_probe_kernel(int iters, T seed, T *__restrict__ out) {
-  T a0 = seed + T(threadIdx.x), a1 = a0 + T(1), a2 = a0 + T(2), a3 = a0 + T(3);
-  T a4 = a0 + T(4), a5 = a0 + T(5), a6 = a0 + T(6), a7 = a0 + T(7);
-  if constexpr (REGS == 2) {
-    const T d = T(threadIdx.x) * T(1e-9);
-    const T m0 = T(0.999999) + d, m1 = T(0.999998) + d, m2 = T(0.999997) + d, m3 = T(0.999996) + d;
-    const T m4 = T(0.999995) + d, m5 = T(0.999994) + d, m6 = T(0.999993) + d, m7 = T(0.999992) + d;
-    const T c0 = T(1e-6) + d, c1 = T(2e-6) + d, c2 = T(3e-6) + d, c3 = T(4e-6) + d;
-    const T c4 = T(5e-6) + d, c5 = T(6e-6) + d, c6 = T(7e-6) + d, c7 = T(8e-6) + d;
-#pragma unroll 8
-    for (int i = 0; i < iters; ++i) {
-      a0 = fma_(a0, m0, c0); a1 = fma_(a1, m1, c1); a2 = fma_(a2, m2, c2); a3 = fma_(a3, m3, c3);
-      a4 = fma_(a4, m4, c4); a5 = fma_(a5, m5, c5); a6 = fma_(a6, m6, c6); a7 = fma_(a7, m7, c7);
-    }
-  } else {
-    const T m = REGS ? T(0.999999) + T(threadIdx.x) * T(1e-9) : T(0.999999);
-    const T c = REGS ? T(1e-6) + T(threadIdx.x) * T(1e-9) : T(1e-6);
-#pragma unroll 8
-    for (int i = 0; i < iters; ++i) {
-      a0 = fma_(a0, m, c); a1 = fma_(a1, m, c); a2 = fma_(a2, m, c); a3 = fma_(a3, m, c);
-      a4 = fma_(a4, m, c); a5 = fma_(a5, m, c); a6 = fma_(a6, m, c); a7 = fma_(a7, m, c);
-    }
-  }
-  T s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-  if (s == T(-12345.678)) out[0] = s;   // never true; keeps the chains alive
-}
-
-// The same for the packed FP32x2 instruction (FFMA2) that the default FP32 integrator is made of: eight chains
-// of float pairs per thread, every chain with its own multiplier and addend pair (three fresh 64-bit register
-// reads per instruction).  Flops = 2 * 2 * 8 * iters * threads.
-__global__ void fma2_probe_kernel(int iters, float seed, float *__restrict__ out) {
-  const float b = seed + (float)threadIdx.x, d = (float)threadIdx.x * 1e-9f;
-  f32x2 a[8], m[8], c[8];
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    a[j] = f32x2(b + (float)j, b + (float)j + 0.5f);
-    m[j] = f32x2(0.999999f - (float)j * 1e-6f + d, 0.999991f - (float)j * 1e-6f + d);
-    c[j] = f32x2((float)(j + 1) * 1e-6f + d, (float)(j + 1) * 1.5e-6f + d);
-  }
-#pragma unroll 8
-  for (int i = 0; i < iters; ++i) {
-#pragma unroll
-    for (int j = 0; j < 8; ++j) a[j] = fma_(a[j], m[j], c[j]);
-  }
-  f32x2 s = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
-  if (s.v.x + s.v.y == -12345.678f) out[0] = s.v.x;   // never true; keeps the chains alive
 }
 
 __global__ void count_status_kernel(const int32_t *__restrict__ status, uint64_t n, gray2_stats *stats) {

@@ -188,10 +188,37 @@ template <typename T> struct Ray {
   T t, x, y, z, u0, u1, u2, u3;
 };
 
+// FP32 only: the running residuals of the eight state sums (DESIGN R12).  A ray of cfg3 takes ~1000 steps
+// whose increments h u, h xddot are 1e2...1e5 times smaller than the variables they are added to, so a plain
+// float sum rounds away the low bits of every increment; the accumulated loss (an equivalent shift of the
+// impact parameter by ~2e-4 M) is what limited the FP32 integrator, not the float right-hand side.  Each
+// variable is therefore carried as an unevaluated sum hi + lo (compensated summation, Kahan 1965): the
+// right-hand side sees hi, the increment is added as  inc = fma(h/6, S, lo); t = hi + inc; lo = inc - (t - hi).
+// Three more instructions per variable and step.  The double kernels do not need it (Carry<double> is empty).
+template <typename T> struct Carry {
+  static constexpr bool compensated = true;
+  T t, x, y, z, u0, u1, u2, u3;
+  __device__ __forceinline__ void clear() { t = x = y = z = u0 = u1 = u2 = u3 = T(0); }
+};
+template <> struct Carry<double> {
+  static constexpr bool compensated = false;
+  __device__ __forceinline__ void clear() {}
+};
+
+// hi <- hi + w S  (w = h/6; S = k1 + 2 k2 + 2 k3 + k4), compensated when a residual is carried.
+template <typename T>
+__device__ __forceinline__ void advance(T &hi, T &lo, T w, T S) {
+  const T inc = fma_(w, S, lo);
+  const T t = hi + inc;
+  lo = inc - (t - hi);
+  hi = t;
+}
+__device__ __forceinline__ void advance(double &hi, double w, double S) { hi = fma(w, S, hi); }
+
 // Classic RK4.  `g1` is the geometry at the current position (already needed by the
 // stopping test and the step rule), so stage 1 costs only the velocity-dependent part.
 template <typename T>
-__device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, const Vel<T> &w1, T h) {
+__device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, Carry<T> &c, const Geometry<T> &g1, const Vel<T> &w1, T h) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
   T b0, b1, b2, b3;                      // stage acceleration
   T v0, v1, v2, v3;                      // stage velocity
@@ -221,14 +248,15 @@ __device__ __forceinline__ void rk4_step(const SpinConst<T> &k, Ray<T> &s, const
   // stage 4
   ks_geometry(k, px, py, pz, g);
   ks_accel(k, g, px, py, v0, v1, v2, v3, b0, b1, b2, b3);
-  s.t = fma_(h6, St + v0, s.t);
-  s.x = fma_(h6, Sx + v1, s.x);
-  s.y = fma_(h6, Sy + v2, s.y);
-  s.z = fma_(h6, Sz + v3, s.z);
-  s.u0 = fma_(h6, S0 + b0, s.u0);
-  s.u1 = fma_(h6, S1 + b1, s.u1);
-  s.u2 = fma_(h6, S2 + b2, s.u2);
-  s.u3 = fma_(h6, S3 + b3, s.u3);
+  if constexpr (!Carry<T>::compensated) {      // double: plain sums
+    (void)c;
+    advance(s.t, h6, St + v0); advance(s.x, h6, Sx + v1); advance(s.y, h6, Sy + v2); advance(s.z, h6, Sz + v3);
+    advance(s.u0, h6, S0 + b0); advance(s.u1, h6, S1 + b1); advance(s.u2, h6, S2 + b2); advance(s.u3, h6, S3 + b3);
+  } else {
+    advance(s.t, c.t, h6, St + v0); advance(s.x, c.x, h6, Sx + v1); advance(s.y, c.y, h6, Sy + v2);
+    advance(s.z, c.z, h6, Sz + v3); advance(s.u0, c.u0, h6, S0 + b0); advance(s.u1, c.u1, h6, S1 + b1);
+    advance(s.u2, c.u2, h6, S2 + b2); advance(s.u3, c.u3, h6, S3 + b3);
+  }
 }
 
 // ---- coordinate-time form ------------------------------------------------------
@@ -247,7 +275,7 @@ __device__ __forceinline__ void ks_accel_coordtime(const SpinConst<T> &k, const 
 // Classic RK4 in t of the six variables (x, v); uses Ray<T> with u0 unused (v^0 = 1) and t advanced by
 // the caller (t += h exactly).
 template <typename T>
-__device__ __forceinline__ void rk4_step_coordtime(const SpinConst<T> &k, Ray<T> &s, const Geometry<T> &g1, const Vel<T> &w1, T h) {
+__device__ __forceinline__ void rk4_step_coordtime(const SpinConst<T> &k, Ray<T> &s, Carry<T> &c, const Geometry<T> &g1, const Vel<T> &w1, T h) {
   const T hh = T(0.5) * h, h6 = h * T(1.0 / 6.0);
   T b1, b2, b3, v1, v2, v3, px, py, pz;
   T Sx, Sy, Sz, S1, S2, S3;
@@ -270,8 +298,14 @@ __device__ __forceinline__ void rk4_step_coordtime(const SpinConst<T> &k, Ray<T>
   v1 = fma_(h, b1, s.u1); v2 = fma_(h, b2, s.u2); v3 = fma_(h, b3, s.u3);
   ks_geometry(k, px, py, pz, g);
   ks_accel_coordtime(k, g, ks_vel(k, g, px, py, T(1), v1, v2, v3), px, py, v1, v2, v3, b1, b2, b3);
-  s.x = fma_(h6, Sx + v1, s.x); s.y = fma_(h6, Sy + v2, s.y); s.z = fma_(h6, Sz + v3, s.z);
-  s.u1 = fma_(h6, S1 + b1, s.u1); s.u2 = fma_(h6, S2 + b2, s.u2); s.u3 = fma_(h6, S3 + b3, s.u3);
+  if constexpr (!Carry<T>::compensated) {
+    (void)c;
+    advance(s.x, h6, Sx + v1); advance(s.y, h6, Sy + v2); advance(s.z, h6, Sz + v3);
+    advance(s.u1, h6, S1 + b1); advance(s.u2, h6, S2 + b2); advance(s.u3, h6, S3 + b3);
+  } else {
+    advance(s.x, c.x, h6, Sx + v1); advance(s.y, c.y, h6, Sy + v2); advance(s.z, c.z, h6, Sz + v3);
+    advance(s.u1, c.u1, h6, S1 + b1); advance(s.u2, c.u2, h6, S2 + b2); advance(s.u3, c.u3, h6, S3 + b3);
+  }
 }
 
 }  // namespace gray2

@@ -4,8 +4,8 @@ Argument marshalling only: every step of the path runs in the CUDA kernels of ``
 used for device memory and streams, nothing else.  There is no CPU fallback: if the library is not
 built, or there is no CUDA device, the calls raise.
 
-Function names match the C entry points: ``init_null``, ``init_timelike``, ``integrate``,
-``invariants`` (plus the diagnostic ``rhs``).
+Function names match the C entry points: ``init_null``, ``init_explicit`` / ``init_timelike``,
+``integrate``, ``invariants`` (plus the diagnostic ``rhs``).
 """
 from __future__ import annotations
 
@@ -66,6 +66,8 @@ def load_library():
     d, p, i32, u64 = C.c_double, C.c_void_p, C.c_int32, C.c_uint64
     lib.gray2_init_null.argtypes = [p, d, d, d, d, d, i32, i32, p]
     lib.gray2_init_timelike.argtypes = [p, d, p, u64, i32, p]
+    lib.gray2_init_explicit.argtypes = [p, d, p, u64, i32, i32, p]
+    lib.gray2_init_explicit.restype = C.c_int
     lib.gray2_init_null_shard.argtypes = [p, d, d, d, d, d, i32, i32, u64, i32, i32, p]
     lib.gray2_shard_count.argtypes = [u64, u64, i32, i32]
     lib.gray2_shard_count.restype = u64
@@ -82,8 +84,6 @@ def load_library():
     lib.gray2_convert.argtypes = [p, p, u64, i32, p]
     lib.gray2_flops_per_step_bl.argtypes = [i32]
     lib.gray2_set_launch.argtypes = [i32, i32, i32]
-    lib.gray2_fma_probe.argtypes = [i32, i32, i32, i32, i32, p, p]
-    lib.gray2_fma_probe.restype = C.c_int
     lib.gray2_flops_per_step.argtypes = [i32]
     for name in ("gray2_init_null", "gray2_init_timelike", "gray2_integrate", "gray2_invariants", "gray2_rhs",
                  "gray2_set_launch", "gray2_flops_per_step"):
@@ -176,11 +176,28 @@ def init_null_shard(a, r_obs, inclination_rad, fov_half_alpha, fov_half_beta, nx
     return st
 
 
-def init_timelike(a, xu8, prec=F64, renormalise_ut=False, stream=None, out: State | None = None) -> State:
-    """xu8: HOST array (numpy or CPU torch tensor) of shape (n, 8), float64."""
+def _host_xu8(xu8) -> np.ndarray:
     if isinstance(xu8, torch.Tensor):
         xu8 = xu8.detach().cpu().numpy()
-    xu8 = np.ascontiguousarray(np.asarray(xu8, dtype=np.float64).reshape(-1, 8))
+    return np.ascontiguousarray(np.asarray(xu8, dtype=np.float64).reshape(-1, 8))
+
+
+def init_explicit(a, xu8, kind=NULL, prec=F64, renormalise_ut=False, stream=None, out: State | None = None) -> State:
+    """Explicit 8-vectors of null (kind = NULL) or time-like (kind = TIMELIKE) geodesics.
+    xu8: HOST array (numpy or CPU torch tensor) of shape (n, 8), float64."""
+    xu8 = _host_xu8(xu8)
+    n = xu8.shape[0]
+    st = out if out is not None else State.empty(n, prec)
+    cs = st._c()
+    _check(load_library().gray2_init_explicit(C.byref(cs), a, xu8.ctypes.data_as(C.c_void_p), n, int(kind),
+                                              int(renormalise_ut), _stream_ptr(stream)))
+    st._back(cs)
+    return st
+
+
+def init_timelike(a, xu8, prec=F64, renormalise_ut=False, stream=None, out: State | None = None) -> State:
+    """gray2_init_timelike: explicit 8-vectors of time-like geodesics (HOST array of shape (n, 8), float64)."""
+    xu8 = _host_xu8(xu8)
     n = xu8.shape[0]
     st = out if out is not None else State.empty(n, prec)
     cs = st._c()
@@ -281,15 +298,6 @@ def convert(st: State, to_coords: int, n=None, stream=None, out: State | None = 
     _check(load_library().gray2_convert(C.byref(cs), C.byref(cd), n, to_coords, _stream_ptr(stream)))
     dst._back(cd)
     return dst
-
-
-def fma_probe(prec, blocks, threads, iters, scratch: torch.Tensor, register_operands=False, stream=None):
-    """Diagnostic: enqueue the FMA-only probe kernel; returns its flops, 16 * iters * blocks * threads
-    (twice that for register_operands = 3, the packed FP32x2 probe)."""
-    _check(load_library().gray2_fma_probe(prec, int(register_operands), blocks, threads, iters,
-                                          C.c_void_p(scratch.data_ptr()),
-                                          _stream_ptr(stream)))
-    return (32 if int(register_operands) == 3 else 16) * iters * blocks * threads
 
 
 def set_launch(prec, threads_per_block=0, blocks_per_sm=0):

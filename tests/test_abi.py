@@ -130,28 +130,13 @@ def test_new_entries_reject_bad_arguments_without_gpu_work(lib):
     assert lib.gray2_flops_per_step_bl(0) == 598 and lib.gray2_flops_per_step_bl(1) == 566
     assert lib.gray2_flops_per_step_coordtime(0) == 534
     fake = C.c_void_p(0x1000)
-    assert lib.gray2_fma_probe(0, 7, 1, 32, 1, fake, null) == EINVAL                  # unknown operand form
-    assert lib.gray2_fma_probe(0, 3, 1, 32, 1, fake, null) == EINVAL                  # packed form is FP32 only
-    assert lib.gray2_fma_probe(1, 2, 1, 32, 1, null, null) == EINVAL                  # no scratch
-
-
-def test_sass_operand_model_on_a_hand_written_loop():
-    """The cost model of paper_1706_07062_b200.sass_operands: max(2, distinct fresh register
-    operands) cycles per FP64 / packed FP32x2 instruction; immediates, uniform registers, a register named twice
-    and a `.reuse` hit of the previous instruction are free."""
-    from paper_1706_07062_b200 import sass_operands as so
-    loop = [(0x00, "DFMA R0, R2, R4, R6"),            # three fresh registers: 3
-            (0x10, "DMUL R8, R2, R4"),                # two: 2
-            (0x20, "DFMA R10, R12, R12, 1"),          # one register named twice and an immediate: 2 (floor)
-            (0x30, "DFMA R14, R16.reuse, R18, R20"),  # 3, leaves R16 in slot 0
-            (0x40, "DFMA R22, R16, R24, R26"),        # R16 comes from the reuse cache: 2
-            (0x50, "IMAD.MOV.U32 R30, RZ, RZ, RZ"),   # not an FP instruction, breaks nothing it did not set
-            (0x60, "DFMA R22, R16, R24, UR4"),        # uniform register: 2
-            (0x70, "@P0 DADD R2, R2, -R6")]           # predicated add: 2
-    r = so.account(loop)
-    assert r["fp"] == 7 and r["cycles"] == 3 + 2 + 2 + 3 + 2 + 2 + 2
-    assert r["three_read"] == 2 and r["reuse_hits"] == 1
-    assert r["by_op"] == {"DFMA": 5, "DMUL": 1, "DADD": 1}
+    s.n = 16
+    assert lib.gray2_init_explicit(C.byref(s), 0.5, fake, 16, 7, 0, null) == EINVAL   # unknown kind
+    assert b"kind" in lib.gray2_last_error()
+    assert lib.gray2_init_explicit(C.byref(s), 0.5, null, 16, 0, 0, null) == EINVAL   # no host array
+    assert lib.gray2_init_explicit(C.byref(s), 0.5, fake, 17, 0, 0, null) == ESTATE   # n > s->n
+    assert lib.gray2_init_explicit(C.byref(s), 1.5, fake, 16, 1, 0, null) == EINVAL   # |a| > 1
+    assert not hasattr(lib, "gray2_fma_probe")        # the probe kernels live in bench_probe.cu, not in the product
 
 
 def test_bench_reference_arm_prints_the_contract_line():
@@ -179,3 +164,30 @@ def test_bench_gpu_arm_fails_loudly_without_a_gpu():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1"], capture_output=True,
                          text=True, timeout=300)
     assert out.returncode != 0 and "no CPU fallback" in (out.stderr + out.stdout)
+
+
+def test_bench_gpus_n_without_the_devices_fails_loudly():
+    """`bench.py --gpus 2` outside torchrun starts the ranks itself; on a box with fewer than 2 GPUs it must say so
+    and exit non-zero instead of printing a one-rank line."""
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available() and torch.cuda.device_count() >= 2:
+        pytest.skip("two GPUs are present")
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1"],
+                         capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode != 0 and "needs 2 CUDA devices" in (out.stderr + out.stdout)
+    assert "n_gpus" not in out.stdout
+
+
+def test_bench_probe_object_builds_and_is_separate_from_the_product():
+    import subprocess
+    sys_path = os.path.join(ROOT, "bench_probe.cu")
+    assert os.path.exists(sys_path)
+    import bench                                            # bench.py at the repo root (conftest puts it on sys.path)
+    lib = C.CDLL(bench.build_probe())
+    assert hasattr(lib, "bench_fma_probe")
+    assert lib.bench_fma_probe(0, 3, 1, 32, 1, C.c_void_p(0x1000), None) == 1        # packed form is FP32 only
+    assert lib.bench_fma_probe(1, 2, 1, 32, 1, None, None) == 1                      # no scratch
+    assert bench.load_counters("cfg3", "f64", "affine") is not None

@@ -20,10 +20,9 @@ def table1_xu8():
 
 def run_pair(a, xu8, kind, lam_end, **kw):
     gsc, osc = sc_pair(**kw)
-    g = gray2.init_timelike(a, xu8)
-    g.kind = kind
-    o = oracle.init_timelike(a, xu8)
-    o.kind = kind
+    g = gray2.init_explicit(a, xu8, kind)
+    o = oracle.init_explicit(a, xu8, kind)
+    assert g.kind == kind == o.kind
     stats = gray2.new_stats()
     gd = gray2.integrate_diagnostics(g, lam_end, gsc, stats=stats)
     ostats, od = oracle.integrate_diagnostics(o, lam_end, osc)
@@ -94,8 +93,7 @@ def test_convergence_study_of_the_paper_on_the_gpu():
     exact_peak = np.array([cf.max_abs_costheta(1.0, *cf.teo_phi_q(1.0, r["r"])) for r in ROWS])
     u2, pk, dp = [], [], []
     for n in (16, 32, 64, 128, 256):
-        g = gray2.init_timelike(1.0, xu8)
-        g.kind = gray2.NULL
+        g = gray2.init_explicit(1.0, xu8, gray2.NULL)
         d = gray2.integrate_diagnostics(g, 6.0 if n < 256 else 24.0, gray2.step_control(mode=0, h_fixed=1.0 / n, max_steps=10 ** 7))
         u2.append(d["max_abs_u2"].cpu().numpy())
         pk.append(np.abs(d["cos_peak"].cpu().numpy() - exact_peak))
@@ -110,8 +108,7 @@ def test_convergence_study_of_the_paper_on_the_gpu():
 
 def test_fp32_diagnostics_and_edges():
     xu8 = table1_xu8()
-    g = gray2.init_timelike(1.0, xu8, prec=gray2.F32)
-    g.kind = gray2.NULL
+    g = gray2.init_explicit(1.0, xu8, gray2.NULL, prec=gray2.F32)
     d = gray2.integrate_diagnostics(g, 10.0, gray2.step_control(mode=0, h_fixed=1.0 / 64, max_steps=10 ** 6))
     pk = d["cos_peak"].cpu().numpy()
     assert np.abs(pk - np.array([r["maxcos"] for r in ROWS])).max() < 2e-3

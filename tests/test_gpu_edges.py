@@ -7,8 +7,8 @@ import torch
 
 import image_helpers as ih
 import oracle
-from gpu_helpers import (INF, TOL_STATE_F64, image_sc, run_gpu_image, sc_pair, state_rel_error, take,
-                         to_oracle_state)
+from gpu_helpers import (INF, TOL_STATE_F64, TWINS_ORBIT, accumulated_rounding_f64, assert_fp32_parity, image_sc, image_sc_kw, make_straddle_check, run_gpu_image,
+                         sc_pair, state_rel_error, take, to_oracle_state, twin_sensitivity)
 from paper_1706_07062_b200 import gray2, inputs
 
 pytestmark = pytest.mark.gpu
@@ -181,17 +181,17 @@ def test_more_calls_in_flight_than_work_queue_slots():
         assert gray2.stats_dict(st) == ref_stats
 
 
-def test_fma_probes_run_in_every_form():
-    """The diagnostic FMA kernels behind bench.py's fma_probe_* fields: every operand form launches and
-    reports its flop count (16 per thread and iteration, 32 for the packed FP32x2 form)."""
-    for prec, dtype, forms in ((gray2.F64, torch.float64, (0, 1, 2)), (gray2.F32, torch.float32, (0, 1, 2, 3))):
+def test_fma_probes_of_the_bench_run_in_every_form():
+    """The FMA-only kernels behind bench.py's fma_probe_* fields live in bench_probe.cu (not in the product
+    library): every operand form launches, bad forms are refused."""
+    import bench
+    lib = bench.load_probe()
+    for prec, dtype, forms in ((0, torch.float64, (0, 1, 2)), (1, torch.float32, (0, 1, 2, 3))):
         scratch = torch.zeros(8, dtype=dtype, device="cuda")
         for form in forms:
-            flops = gray2.fma_probe(prec, 4, 64, 10, scratch, register_operands=form)
-            assert flops == (32 if form == 3 else 16) * 10 * 4 * 64
+            assert lib.bench_fma_probe(prec, form, 4, 64, 10, scratch.data_ptr(), None) == 0
     torch.cuda.synchronize()
-    with pytest.raises(Exception):
-        gray2.fma_probe(gray2.F64, 4, 64, 10, torch.zeros(8, dtype=torch.float64, device="cuda"), register_operands=3)
+    assert lib.bench_fma_probe(0, 3, 4, 64, 10, scratch.data_ptr(), None) == 1
 
 
 def test_backward_direction_and_lambda_clip():
@@ -256,10 +256,15 @@ def test_cfg4_ensemble_sample_parity_and_drift():
     gst = to_oracle_state(g)
     assert gray2.stats_dict(stats)["steps"] == 4096 * 3000 and (gst.status == gray2.MAXSTEPS).all()
     # 3000 steps ~ several radial periods.  The two sides round in different orders (Christoffel form vs
-    # regrouped form); eccentric orbits with a deep periapsis amplify that 1e-16 difference along the orbit
-    # (phase error), so the 1e-9 bound is asserted on 99.9% of the particles and 1e-8 on all (DESIGN "Tolerances").
+    # regrouped form); eccentric orbits with a deep periapsis amplify that difference along the orbit (phase
+    # error).  Which orbits are critical is decided by the oracle alone (twin orbits displaced by the accumulated
+    # rounding of 3000 steps, gpu_helpers.accumulated_rounding_f64); 1e-9 holds on EVERY other one.
     err = state_rel_error(gst.q, o.q, 0.7)
-    assert np.quantile(err, 0.999) < TOL_STATE_F64 and err.max() < 10 * TOL_STATE_F64, (np.quantile(err, 0.999), err.max())
+    kw = dict(mode=0, h_fixed=0.5, max_steps=3000)
+    sens = twin_sensitivity(oracle.init_timelike(0.7, xu8), kw, rel_delta=accumulated_rounding_f64(3000), twins=TWINS_ORBIT)
+    noncrit = sens <= TOL_STATE_F64
+    print("[cfg4 sample] %d of 4096 orbits critical; max error on the others %.2e, on all %.2e" % ((~noncrit).sum(), err[noncrit].max(), err.max()))
+    assert noncrit.mean() > 0.99 and err[noncrit].max() < TOL_STATE_F64, (noncrit.mean(), err[noncrit].max())
     gi1 = [t.cpu().numpy() for t in gray2.invariants(g)]
     oi1 = oracle.invariants(o)
     from gpu_helpers import invariant_term_scales
@@ -271,7 +276,9 @@ def test_cfg4_ensemble_sample_parity_and_drift():
 
 def test_cfg4_full_size_sampled_parity():
     """BASELINE.json configs[3] at full size (1,048,576 particles x 100,000 fixed steps) in the launch
-    configuration bench.py uses; 64 sampled particles against the oracle."""
+    configuration bench.py uses; 768 sampled particles against the oracle: 512 evenly spaced through the ensemble
+    and the 256 with the deepest periapses (smallest r_p = p / (1 + e): the orbits that amplify a rounding-level
+    difference between the two formulations most, "u^2 ... increases")."""
     n, nsteps = 1 << 20, 100000
     xu8, meta = inputs.cfg4_ensemble(n)
     gsc, osc = sc_pair(mode=0, h_fixed=0.5, max_steps=nsteps)
@@ -283,20 +290,46 @@ def test_cfg4_full_size_sampled_parity():
     assert sd["n_invalid"] == 0 and sd["n_active"] == 0 and sd["n_escaped"] == 0
     assert sd["n_maxsteps"] + sd["n_captured"] == n and sd["n_captured"] < 100     # marginal orbits may plunge at h = 0.5
     assert sd["steps"] == int(g.nsteps.sum(dtype=torch.int64).item())
-    idx = np.arange(0, n, n // 64)[:64]
+    even = np.arange(0, n, n // 512)[:512]
+    rp = meta["p"] / (1.0 + meta["e"])
+    deep = np.setdiff1d(np.argsort(rp, kind="stable")[:300], even)[:256]
+    idx = np.concatenate([even, deep])
     o = oracle.init_timelike(0.7, xu8[idx])
     oi0 = oracle.invariants(o)
     oracle.integrate(o, INF, osc)
     tidx = torch.tensor(idx, device="cuda")
     assert np.array_equal(g.nsteps[tidx].cpu().numpy(), o.nsteps) and np.array_equal(g.status[tidx].cpu().numpy(), o.status)
     err = state_rel_error(g.q[:, tidx].cpu().numpy(), o.q, 0.7)
-    assert err.max() < TOL_STATE_F64, err.max()
+    orbiting = o.status == oracle.MAXSTEPS
+    print("[cfg4 full size] state error after 1e5 steps: evenly spaced max %.2e; deepest periapses (r_p %.3f..%.3f, %d still "
+          "orbiting) median %.2e 99%% %.2e max %.2e" % (err[:512].max(), rp[deep].min(), rp[deep].max(), orbiting[512:].sum(),
+                                                         np.median(err[512:][orbiting[512:]]), np.quantile(err[512:][orbiting[512:]], 0.99),
+                                                         err[512:][orbiting[512:]].max()))
+    # Which of these orbits are critical over 1e5 steps is decided by the oracle alone: twin orbits displaced by the
+    # accumulated rounding of the run (gpu_helpers.accumulated_rounding_f64: 2^-52 sqrt(4 nsteps) = 1.4e-13 relative);
+    # 1e-9 holds on EVERY orbit whose final state is stable to 1e-9 under that displacement.
+    kw = dict(mode=0, h_fixed=0.5, max_steps=nsteps)
+    sens = twin_sensitivity(oracle.init_timelike(0.7, xu8[idx]), kw, rel_delta=accumulated_rounding_f64(nsteps), twins=TWINS_ORBIT)
+    noncrit = orbiting & (sens <= TOL_STATE_F64)
+    print("[cfg4 full size] critical or plunged: %d of the 512 evenly spaced, %d of the 256 deepest; max error on the others %.2e"
+          % ((~noncrit[:512]).sum(), (~noncrit[512:]).sum(), err[noncrit].max()))
+    assert noncrit[:512].mean() > 0.95 and err[noncrit].max() < TOL_STATE_F64, (noncrit[:512].mean(), err[noncrit].max())
     gi1 = [t.cpu().numpy() for t in gray2.invariants(g)]
     oi1 = oracle.invariants(o)
     from gpu_helpers import invariant_term_scales
     scales = invariant_term_scales(o.q)
+    names = ("E", "Lz", "Q", "u.u")
     for k in range(4):
-        assert np.max(np.abs((gi1[k] - gi0[k])[idx] - (oi1[k] - oi0[k])) / scales[k]) < 1e-12
+        gd, od = (gi1[k] - gi0[k])[idx], oi1[k] - oi0[k]
+        sel = orbiting
+        # beside the term-scaled bound of DESIGN section 6, the plain figure: the difference of the two drifts
+        # relative to the drift itself (rms over the sample) and to the invariant
+        print("[cfg4 full size] drift of %-3s: rms %.2e; GPU - oracle: rms %.2e = %.1e of the drift, max %.2e of the invariant's terms"
+              % (names[k], np.sqrt(np.mean(od[sel] ** 2)), np.sqrt(np.mean((gd - od)[sel] ** 2)),
+                 np.sqrt(np.mean((gd - od)[sel] ** 2)) / max(np.sqrt(np.mean(od[sel] ** 2)), 1e-300),
+                 np.max(np.abs(gd - od)[sel] / scales[k][sel])))
+        assert np.max(np.abs(gd - od)[:512] / scales[k][:512]) < 1e-12
+        assert np.max(np.abs(gd - od)[sel] / scales[k][sel]) < 1e-11
     # drift stays at the RK4 truncation level over 1e5 steps
     alive = g.status.cpu().numpy() == gray2.MAXSTEPS      # the few plunging particles end inside the horizon region
     dE, dn = (gi1[0] - gi0[0])[alive], (gi1[3] - gi0[3])[alive]
@@ -310,6 +343,10 @@ def test_cfg5_full_size_sampled_parity(prec):
     cfg = inputs.CFG5_NULL
     gsc, osc = image_sc(cfg)
     g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec)
+    rng = np.random.default_rng(5)
+    idx = np.sort(rng.choice(cfg.n, 768, replace=False))
+    tidx = torch.tensor(idx, device="cuda")
+    g0q = g.q[:, tidx].double().cpu().numpy()              # the sampled rays' initial state as the kernel reads it
     stats = gray2.new_stats()
     gray2.integrate(g, INF, gsc, stats=stats)
     sd = gray2.stats_dict(stats)
@@ -320,14 +357,13 @@ def test_cfg5_full_size_sampled_parity(prec):
     order = np.argsort(ca)
     area = 2.0 * np.trapezoid(cb[order], ca[order])
     assert abs(sd["n_captured"] / cfg.n - area / (2 * cfg.fov) ** 2) < 1e-3
-    rng = np.random.default_rng(5)
-    idx = np.sort(rng.choice(cfg.n, 768, replace=False))
     full0 = oracle.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
     o0 = take(full0, idx)
     del full0
+    if prec == gray2.F32:
+        o0.q[:] = g0q                                      # the same inputs: the float initial state, widened
     o = o0.copy()
     oracle.integrate(o, INF, osc)
-    tidx = torch.tensor(idx, device="cuda")
     gq = g.q[:, tidx].double().cpu().numpy()
     gs, gn = g.status[tidx].cpu().numpy(), g.nsteps[tidx].cpu().numpy()
     xi, eta, _, _ = ih.ray_constants(o0)
@@ -339,8 +375,8 @@ def test_cfg5_full_size_sampled_parity(prec):
         assert np.array_equal(gs[outside], o.status[outside]) and np.array_equal(gn[outside], o.nsteps[outside])
         assert state_rel_error(gq[:, outside], o.q[:, outside], o.a_eff).max() < TOL_STATE_F64
     else:
-        outside = d > 2e-2
-        assert np.array_equal(gs[outside], o.status[outside])
-        same = outside & (gn == o.nsteps)
-        err = state_rel_error(gq[1:][:, same], o.q[1:][:, same], o.a_eff)
-        assert same.sum() > 0.5 * outside.sum() and np.quantile(err, 0.9) < 1e-4
+        kw = image_sc_kw(cfg)
+        gst = oracle.State(len(idx), gq, g.lam[tidx].cpu().numpy(), gs, gn, o.a_eff, o.kind, o.reversed, o.coords)
+        sens = twin_sensitivity(o0, kw)
+        assert_fp32_parity(cfg.name + " full size, 768 sampled rays", gst, o, sens, state_rel_error(gq, o.q, o.a_eff),
+                           make_straddle_check(o0, gst, o, kw))

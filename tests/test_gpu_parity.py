@@ -6,8 +6,9 @@ import torch
 
 import image_helpers as ih
 import oracle
-from gpu_helpers import (INF, invariant_term_scales, TOL_DRIFT_F64, TOL_STATE_F32, TOL_STATE_F64, drift, gpu_invariants_np, image_sc,
-                         run_gpu_image, run_oracle_image, sc_pair, state_rel_error, take, to_oracle_state)
+from gpu_helpers import (INF, invariant_term_scales, TOL_DRIFT_F64, TOL_STATE_F32, TOL_STATE_F64, assert_fp32_parity, drift,
+                         gpu_invariants_np, image_sc, image_sc_kw, make_straddle_check, run_gpu_image, run_oracle_image, sc_pair,
+                         state_rel_error, take, to_oracle_state, twin_sensitivity)
 from paper_1706_07062_b200 import gray2, inputs
 
 pytestmark = pytest.mark.gpu
@@ -144,20 +145,66 @@ def test_kerr_images_reduced_resolution_full_parity(cfg):
     assert abs(gstats["steps"] - ostats["steps"]) <= 40 * (~outside).sum()
 
 
-@pytest.mark.parametrize("cfg", [inputs.CFG3_NULL.scaled(64), inputs.CFG1_NULL], ids=lambda c: c.name)
+@pytest.mark.parametrize("cfg", [inputs.CFG3_NULL.scaled(64), inputs.CFG1_NULL, inputs.CFG2_NULL.scaled(72, 56)],
+                         ids=lambda c: c.name)
 def test_fp32_against_oracle(cfg):
+    """north_star's FP32 clause on EVERY non-critical ray, all eight components (DESIGN R12; gpu_helpers)."""
     g0, g, gstats = run_gpu_image(cfg, prec=gray2.F32)
-    o0, o, _ = run_oracle_image(cfg)
+    o0 = to_oracle_state(g0)                        # the same inputs: the float initial state, widened
+    o = o0.copy()
+    kw = image_sc_kw(cfg)
+    oracle.integrate(o, INF, oracle.step_control(**kw))
     gst = to_oracle_state(g)
-    d, mask = ih.classify_image(cfg, o0)
-    outside = d > 1e-3 * 20          # FP32 rounding of the pixel position alone is ~1e-4 M at r_obs = 1000
-    assert np.array_equal((gst.status == gray2.CAPTURED)[outside], mask[outside])
-    same = outside & (gst.nsteps == o.nsteps) & (gst.status == o.status)
-    assert same.sum() > 0.5 * outside.sum()
-    err = state_rel_error(gst.q[1:][:, same], o.q[1:][:, same], o.a_eff)
-    # bulk of the rays within the stated tolerance; the few strongly lensed ones amplify FP32 rounding
-    assert np.quantile(err, 0.90) < TOL_STATE_F32, np.quantile(err, [0.5, 0.9, 0.99, 1.0])
-    assert np.median(err) < 0.2 * TOL_STATE_F32
+    sens = twin_sensitivity(o0, kw)
+    err = state_rel_error(gst.q, o.q, o.a_eff)
+    noncrit, same = assert_fp32_parity(cfg.name, gst, o, sens, err, make_straddle_check(o0, gst, o, kw))
+    # the capture mask against Carter's potential, from the constants of the rounded input
+    xi, eta, _, _ = ih.ray_constants(o0)
+    mask = ih.potential_mask(o0.a_eff, xi, eta, 0.9 * cfg.r_obs)
+    assert np.array_equal((gst.status == gray2.CAPTURED)[noncrit], mask[noncrit])
+    assert gstats["n_active"] == 0 and gstats["n_invalid"] == 0
+
+
+def degenerate_band_distance(cfg, o0):
+    """Distance of every ray to the critical curve in the asymptotic image plane for the cases the general band
+    machinery does not cover (it needs sin i != 0 and |a| < 1), from closed forms and the ray constants
+    (xi, eta) of the oracle's initial state:
+      face-on (sin i = 0): every ray has xi = 0 and the picture is axisymmetric, so the curve is the circle of
+        radius sqrt(eta_c + a^2), eta_c = Q(r_0) at the spherical photon orbit with Phi(r_0) = 0 (a = 0: sqrt 27),
+        and a ray sits at radius sqrt(eta + a^2);
+      extremal spin: Phi(r) = -(r^2 - 2r - 1), Q(r) = -r^3 (r - 4) for 1 < r <= 4, plus the vertical segment
+        alpha = -2 / sin i, |beta| <= sqrt(3 + cos^2 i - 4 cot^2 i), onto which all of r -> 1 is mapped."""
+    import closed_forms as cf
+    xi, eta, _, _ = ih.ray_constants(o0)
+    a, inc = abs(cfg.a), cfg.inclination
+    if abs(np.sin(inc)) < 1e-12:
+        assert np.abs(xi).max() < 1e-9
+        if a == 0.0:
+            rc = np.sqrt(27.0)
+        else:
+            lo, hi = cf.r_photon_prograde(a), cf.r_photon_retrograde(a)
+            for _ in range(200):                        # bisection on Phi(r) = 0
+                mid = 0.5 * (lo + hi)
+                lo, hi = (mid, hi) if cf.teo_phi_q(a, mid)[0] > 0 else (lo, mid)
+            rc = np.sqrt(cf.teo_phi_q(a, lo)[1] + a * a)
+        return np.abs(np.sqrt(np.maximum(eta + a * a, 0.0)) - rc)
+    assert a == 1.0
+    r = np.linspace(1.0, 4.0, 400001)[1:]
+    cxi, ceta = -(r * r - 2 * r - 1), -r ** 3 * (r - 4)
+    b2 = ceta + np.cos(inc) ** 2 - cxi ** 2 / np.tan(inc) ** 2
+    ca, cb = -cxi[b2 >= 0] / np.sin(inc), np.sqrt(b2[b2 >= 0])
+    seg = np.sqrt(max(3.0 + np.cos(inc) ** 2 - 4.0 / np.tan(inc) ** 2, 0.0))
+    ca = np.concatenate([ca, np.full(20001, -2.0 / np.sin(inc))])
+    cb = np.concatenate([cb, np.linspace(0.0, seg, 20001)])
+    _, beta = ih.pixel_grid(cfg)
+    al, be = ih.asymptotic_image_point(o0.a_eff, inc, xi, eta, np.where(beta >= 0, 1.0, -1.0))
+    if cfg.a < 0:
+        ca = -ca
+    d = np.empty(al.size)
+    for lo in range(0, al.size, 256):
+        hi = min(lo + 256, al.size)
+        d[lo:hi] = np.sqrt(np.min((ca[None, :] - al[lo:hi, None]) ** 2 + (cb[None, :] - np.abs(be[lo:hi, None])) ** 2, axis=1))
+    return d
 
 
 @pytest.mark.parametrize("a,inc_deg", [(1.0, 80.0), (0.9375, 0.0), (-0.99, 180.0), (0.0, 0.0)],
@@ -165,15 +212,20 @@ def test_fp32_against_oracle(cfg):
 def test_degenerate_geometries(a, inc_deg):
     """Extremal spin, and the face-on view in which the rays run along the spin axis through the poles
     (the case that crashes Boyer-Lindquist integrators): no special handling exists or is
-    needed.  The band machinery needs sin(i) != 0 and |a| < 1, so agreement is asserted on every ray whose
-    step count equals the oracle's, and those must be all but a handful of near-critical rays."""
+    needed.  Status and step count must equal the oracle's on EVERY ray further than 1e-3 M from the critical
+    curve (closed forms for these four cases: degenerate_band_distance), the states to 1e-9."""
     cfg = inputs.NullImageConfig("t", a, 1000.0, inc_deg, 9.0, 64, 48)
     g0, g, gstats = run_gpu_image(cfg)
     o0, o, ostats = run_oracle_image(cfg)
     gst = to_oracle_state(g)
-    same = (gst.nsteps == o.nsteps) & (gst.status == o.status)
-    assert same.mean() > 0.995, same.mean()
-    assert (gst.status == o.status).mean() > 0.999
+    d = degenerate_band_distance(cfg, o0)
+    outside = d > 1e-3
+    assert outside.mean() > 0.99, outside.mean()
+    assert np.array_equal(gst.status[outside], o.status[outside])
+    assert np.array_equal(gst.nsteps[outside], o.nsteps[outside])
+    differ = (gst.nsteps != o.nsteps) | (gst.status != o.status)
+    print("[degenerate %s] %d rays inside the band, %d of them differ from the oracle" % (cfg.name, (~outside).sum(), differ.sum()))
+    same = ~differ
     assert state_rel_error(gst.q[:, same], o.q[:, same], o.a_eff).max() < TOL_STATE_F64
     assert gstats["n_invalid"] == 0 and gstats["n_active"] == 0 and gstats["n_maxsteps"] == ostats["n_maxsteps"]
     if inc_deg in (0.0, 180.0):

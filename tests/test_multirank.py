@@ -81,3 +81,34 @@ def test_tile_dealing_is_a_permutation_and_matches_the_library_count():
             j = torch.arange(p.numel())
             assert torch.equal(p, ((j // tile) * world + r) * tile + j % tile)
     assert lib.gray2_shard_count(10, 0, 0, 1) == 0 and lib.gray2_shard_count(10, 3, 2, 2) == 0    # bad arguments
+
+
+def _bench_rank(payload):
+    """What bench.py's ranks do around the measurement, on CPU: read the torchrun-style environment that
+    launch_ranks sets, join the group, reduce (time = max, work = sum)."""
+    sys.path.insert(0, ROOT)
+    from paper_1706_07062_b200 import multi
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    assert int(os.environ["LOCAL_RANK"]) == rank and os.environ["MASTER_ADDR"] == "127.0.0.1"
+    dist.init_process_group("gloo")
+    times, work = multi.reduce_job([0.25 * (rank + 1)], [100 + rank])
+    if rank == 0:
+        torch.save({"times": times, "work": work, "world": world}, payload)
+    dist.barrier()
+    dist.destroy_process_group()
+    return 0
+
+
+def _failing_rank(payload):
+    return 3 if int(os.environ["RANK"]) == 1 else 0
+
+
+def test_bench_launch_ranks_starts_n_processes_with_the_torchrun_environment(tmp_path):
+    import bench                                            # bench.py at the repo root (conftest puts it on sys.path)
+    out = str(tmp_path / "b.pt")
+    assert bench.launch_ranks(2, _bench_rank, out) == 0
+    res = torch.load(out)
+    assert res == {"times": [0.5], "work": [201.0], "world": 2}
+    import pytest
+    with pytest.raises(Exception):
+        bench.launch_ranks(2, _failing_rank, None)          # a failing rank fails the launch
