@@ -78,6 +78,11 @@ typedef struct {
   int32_t  reversed;    /* 1: time-reversed ray of a backward trace (physical t = -t, L_z = -L_z)       */
   int32_t  coords;      /* gray2_coords of q[]; set to GRAY2_KS by gray2_init_*, to the target by         */
                         /* gray2_convert; gray2_integrate and gray2_invariants follow it                  */
+  const int32_t *order; /* optional (NULL = none): DEVICE array of n int32, a permutation of 0..n-1.  The   */
+                        /* integrators hand geodesic order[k] to the k-th lane that asks for work (SURVEY   */
+                        /* 8(a) a6, 8(b): "optional order array").  It changes the schedule only -- no       */
+                        /* output bit depends on it -- and is used only by calls that cover all n geodesics.  */
+                        /* Longest first shortens the tail of a launch (gray2_order_longest_first).           */
 } gray2_state;
 
 /* Step and stopping rule (DESIGN R4-R6).  For every geodesic with status ACTIVE, repeat:
@@ -210,6 +215,14 @@ int gray2_integrate_diagnostics(gray2_state *s, uint64_t n, double lambda_end, c
  * E, Lz, Q, norm: DEVICE arrays of n doubles each. */
 int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, double *Q, double *norm,
                      void *cuda_stream);
+
+/* Longest-first schedule from a previous trace of the same (or a similar) batch: order <- the indices 0..n-1
+ * sorted by decreasing steps_hint[k] (e.g. the nsteps array an earlier gray2_integrate left for the same image:
+ * movie frames, parameter scans).  Counting sort on the device, 4096 bins over [0, max hint]; the order inside a
+ * bin is unspecified (it cannot change a result).  The paper's kernel pays the whole tail -- every ray runs until
+ * the slowest one of the image is done; with per-ray termination the tail is the last ray of
+ * every lane, and it is shortest when the short rays come last.  steps_hint, order: DEVICE arrays of n int32. */
+int gray2_order_longest_first(const int32_t *steps_hint, uint64_t n, int32_t *order, void *cuda_stream);
 
 /* Optional tuning of gray2_integrate's launch (0 = library default).  Results never depend on it. */
 int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm);

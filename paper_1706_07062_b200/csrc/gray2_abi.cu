@@ -39,6 +39,8 @@ int fail(int code, const char *fmt, ...) {
 constexpr int kQueueSlots = 64;
 constexpr int kMaxDevices = 64;
 struct Scratch {
+  unsigned *order_bins = nullptr;            // device, 2 * kOrderBins + 1 words (gray2_order_longest_first)
+  cudaEvent_t order_done = nullptr;          // recorded behind its last user
   unsigned long long *queue = nullptr;       // device, kQueueSlots * 8 words
   cudaEvent_t done[kQueueSlots] = {};        // recorded behind the last work that used the slot
   unsigned next = 0;
@@ -122,12 +124,13 @@ cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::Step
   uint64_t cap = (uint64_t)num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<T>(s);
+  const int32_t *order = n == s->n ? s->order : nullptr;      // a schedule covers the whole state or is not used
   if (p.mode == 1) {
-    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
-    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
   } else {
-    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
-    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
   }
   return cudaGetLastError();
 }
@@ -140,12 +143,13 @@ cudaError_t launch_integrate_x2(const gray2_state *s, uint64_t n, const gray2::S
   uint64_t cap = (uint64_t)num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<float>(s);
+  const int32_t *order = n == s->n ? s->order : nullptr;
   if (p.mode == 1) {
-    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
-    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
   } else {
-    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
-    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
   }
   return cudaGetLastError();
 }
@@ -568,6 +572,36 @@ int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 534; }
  *   rest of the right-hand side 81 (4 of them reciprocals)  ->  124 / 116 per right-hand side
  *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 598 / 566 per step. */
 int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 566 : 598; }
+
+int gray2_order_longest_first(const int32_t *steps_hint, uint64_t n, int32_t *order, void *cuda_stream) {
+  if (!steps_hint || !order || n == 0) return fail(GRAY2_EINVAL, "gray2_order_longest_first: NULL pointer or n == 0");
+  if (n > 0x7fffffffull) return fail(GRAY2_EINVAL, "gray2_order_longest_first: n exceeds the range of an int32 index");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return fail(GRAY2_ECUDA, "device ordinal %d out of range", dev);
+  constexpr int bins = gray2::kOrderBins;
+  std::lock_guard<std::mutex> guard(g_scratch_lock);        // one histogram per device: calls are serialised
+  Scratch &sc = g_scratch[dev];
+  if (!sc.order_bins) {
+    CUDA_TRY(cudaMalloc(&sc.order_bins, (2 * bins + 1) * sizeof(unsigned)));
+    CUDA_TRY(cudaEventCreateWithFlags(&sc.order_done, cudaEventDisableTiming));
+  }
+  int sms = 0;
+  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  unsigned *hist = sc.order_bins, *cursor = hist + bins, *kmax = hist + 2 * bins;
+  unsigned grid = (unsigned)((n + 255) / 256);
+  if (grid > (unsigned)(sms * 8)) grid = (unsigned)(sms * 8);
+  CUDA_TRY(cudaStreamWaitEvent(st, sc.order_done, 0));       // the previous user of the histogram, on any stream
+  CUDA_TRY(cudaMemsetAsync(hist, 0, (2 * bins + 1) * sizeof(unsigned), st));
+  gray2::order_max_kernel<<<grid, 256, 0, st>>>(steps_hint, n, kmax);
+  gray2::order_hist_kernel<<<grid, 256, 0, st>>>(steps_hint, n, kmax, hist);
+  gray2::order_scan_kernel<<<1, bins / 4, 0, st>>>(hist, cursor);
+  gray2::order_scatter_kernel<<<grid, 256, 0, st>>>(steps_hint, n, kmax, cursor, order);
+  CUDA_TRY(cudaGetLastError());
+  CUDA_TRY(cudaEventRecord(sc.order_done, st));
+  return GRAY2_OK;
+}
 
 int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm) {
   if (prec != GRAY2_F64 && prec != GRAY2_F32) return fail(GRAY2_EINVAL, "gray2_set_launch: unknown precision");

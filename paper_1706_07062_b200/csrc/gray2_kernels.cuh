@@ -105,8 +105,8 @@ __global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ 
 // its derivatives, the radius of the step rule and of the stopping tests is the coordinate r itself.
 template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
-integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long *queue,
-                 unsigned long long *steps_out) {
+integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, const int32_t *__restrict__ order,
+                 unsigned long long *queue, unsigned long long *steps_out) {
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
   const SpinConst<T> k = p.k;
@@ -136,21 +136,32 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
       base = __shfl_sync(0xffffffffu, base, leader);
       if (base + cnt >= n) drained = true;
       if (!have) {
-        uint64_t mine = base + __popc(idle & lt_mask);
-        if (mine < n && s.status[mine] == GRAY2_ACTIVE) {
-          idx = mine;
-          ray.t = s.q[0][idx]; ray.x = s.q[1][idx]; ray.y = s.q[2][idx]; ray.z = s.q[3][idx];
-          ray.u0 = s.q[4][idx]; ray.u1 = s.q[5][idx]; ray.u2 = s.q[6][idx]; ray.u3 = s.q[7][idx];
-          if constexpr (FORM == 1) {
-            lam = (double)ray.t;
-            T w = fastmath<T>::rcp(ray.u0);
-            ray.u1 *= w; ray.u2 *= w; ray.u3 *= w; ray.u0 = T(1);
-          } else {
-            lam = s.lambda[idx];
+        uint64_t mine = base + __popc(idle & lt_mask);      // position in the queue
+        if (mine < n) {
+          if (order) mine = (uint64_t)order[mine];          // ... and the geodesic the caller's schedule puts there
+          // the status and the state are fetched together (one round trip to memory instead of two); an entry
+          // that turns out not to be ACTIVE is dropped and its slot of the lane refilled at the next pass
+          const int32_t st_in = s.status[mine];
+          Ray<T> in;
+          in.t = s.q[0][mine]; in.x = s.q[1][mine]; in.y = s.q[2][mine]; in.z = s.q[3][mine];
+          in.u0 = s.q[4][mine]; in.u1 = s.q[5][mine]; in.u2 = s.q[6][mine]; in.u3 = s.q[7][mine];
+          double lam_in = 0.0;
+          if constexpr (FORM != 1) lam_in = s.lambda[mine];
+          const int32_t nst_in = s.nsteps[mine];
+          if (st_in == GRAY2_ACTIVE) {
+            idx = mine;
+            ray = in;
+            if constexpr (FORM == 1) {
+              lam = (double)ray.t;
+              T w = fastmath<T>::rcp(ray.u0);
+              ray.u1 *= w; ray.u2 *= w; ray.u3 *= w; ray.u0 = T(1);
+            } else {
+              lam = lam_in;
+            }
+            nst = nst0 = nst_in;
+            car.clear();
+            have = true;
           }
-          nst = nst0 = s.nsteps[idx];
-          car.clear();
-          have = true;
         }
       }
       continue;   // entries that were not ACTIVE leave the lane idle: ask again
@@ -235,22 +246,30 @@ struct PairSlot {
 };
 
 template <int C, int FORM>
-__device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, uint64_t mine, Ray<f32x2> &ray,
-                                          Carry<f32x2> &car, PairSlot &sl) {
-  if (mine < n && s.status[mine] == GRAY2_ACTIVE) {
+__device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, const int32_t *__restrict__ order,
+                                          uint64_t mine, Ray<f32x2> &ray, Carry<f32x2> &car, PairSlot &sl) {
+  if (mine >= n) return;
+  if (order) mine = (uint64_t)order[mine];
+  // the status and the state are fetched together (one round trip to memory instead of two)
+  const int32_t st_in = s.status[mine];
+  float t = s.q[0][mine], x = s.q[1][mine], y = s.q[2][mine], z = s.q[3][mine];
+  float u0 = s.q[4][mine], u1 = s.q[5][mine], u2 = s.q[6][mine], u3 = s.q[7][mine];
+  double lam_in = 0.0;
+  if (FORM != 1) lam_in = s.lambda[mine];
+  const int32_t nst_in = s.nsteps[mine];
+  if (st_in == GRAY2_ACTIVE) {
     sl.idx = mine;
-    float t = s.q[0][mine], u0 = s.q[4][mine], u1 = s.q[5][mine], u2 = s.q[6][mine], u3 = s.q[7][mine];
     if (FORM == 1) {
       sl.lam = (double)t;
       float w = fastmath<float>::rcp(u0);
       u1 *= w; u2 *= w; u3 *= w; u0 = 1.0f;
     } else {
-      sl.lam = s.lambda[mine];
+      sl.lam = lam_in;
     }
-    set_half<C>(ray.t, t); set_half<C>(ray.x, s.q[1][mine]); set_half<C>(ray.y, s.q[2][mine]);
-    set_half<C>(ray.z, s.q[3][mine]); set_half<C>(ray.u0, u0); set_half<C>(ray.u1, u1);
+    set_half<C>(ray.t, t); set_half<C>(ray.x, x); set_half<C>(ray.y, y);
+    set_half<C>(ray.z, z); set_half<C>(ray.u0, u0); set_half<C>(ray.u1, u1);
     set_half<C>(ray.u2, u2); set_half<C>(ray.u3, u3);
-    sl.nst = sl.nst0 = s.nsteps[mine];
+    sl.nst = sl.nst0 = nst_in;
     clear_half<C>(car);
     sl.have = true;
     sl.cap = false;
@@ -290,8 +309,8 @@ __device__ __forceinline__ void store_slot(const StateView<float> &s, const Step
 
 template <int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
-integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsigned long long *queue,
-                       unsigned long long *steps_out) {
+integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, const int32_t *__restrict__ order,
+                       unsigned long long *queue, unsigned long long *steps_out) {
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
   const SpinConst<f32x2> k{f32x2(p.k.a), f32x2(p.k.a2), f32x2(p.k.two_a), f32x2(p.k.two_a2), f32x2(p.k.four_a2)};
@@ -314,8 +333,8 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsi
       if (lane == 0) base = atomicAdd(queue, (unsigned long long)cnt);
       base = __shfl_sync(0xffffffffu, base, 0);
       if (base + cnt >= n) drained = true;
-      if (!A.have) load_slot<0, FORM>(s, n, base + __popc(idleA & lt_mask), ray, car, A);
-      if (!B.have) load_slot<1, FORM>(s, n, base + cntA + __popc(idleB & lt_mask), ray, car, B);
+      if (!A.have) load_slot<0, FORM>(s, n, order, base + __popc(idleA & lt_mask), ray, car, A);
+      if (!B.have) load_slot<1, FORM>(s, n, order, base + cntA + __popc(idleB & lt_mask), ray, car, B);
       continue;
     }
     if ((idleA & idleB) == 0xffffffffu) break;
@@ -600,6 +619,56 @@ __global__ void rhs_kernel(SpinConst<T> k, uint64_t n, const T *__restrict__ pos
   T a0, a1, a2, a3;
   ks_accel(k, g, pos[i], pos[n + i], u[i], u[n + i], u[2 * n + i], u[3 * n + i], a0, a1, a2, a3);
   out[i] = a0; out[n + i] = a1; out[2 * n + i] = a2; out[3 * n + i] = a3;
+}
+
+// ---- longest-first schedule (gray2_order_longest_first): counting sort of the indices by decreasing key ----
+constexpr int kOrderBins = 4096;
+
+__global__ void order_max_kernel(const int32_t *__restrict__ key, uint64_t n, unsigned *kmax) {
+  unsigned m = 0;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
+    m = max(m, (unsigned)max(key[i], 0));
+  for (int off = 16; off > 0; off >>= 1) m = max(m, __shfl_down_sync(0xffffffffu, m, off));
+  if ((threadIdx.x & 31) == 0 && m) atomicMax(kmax, m);
+}
+
+__device__ __forceinline__ unsigned order_bin(int32_t key, unsigned kmax) {
+  // bin 0 holds the largest keys; width = ceil((kmax + 1) / bins)
+  const unsigned width = kmax / kOrderBins + 1;
+  return (kmax - min((unsigned)max(key, 0), kmax)) / width;
+}
+
+__global__ void order_hist_kernel(const int32_t *__restrict__ key, uint64_t n, const unsigned *kmax, unsigned *hist) {
+  const unsigned km = *kmax;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
+    atomicAdd(&hist[order_bin(key[i], km)], 1u);
+}
+
+// one block of kOrderBins / 4 threads: exclusive prefix sum of the histogram -> the cursor of every bin
+__global__ void order_scan_kernel(const unsigned *__restrict__ hist, unsigned *cursor) {
+  __shared__ unsigned part[kOrderBins / 4];
+  const unsigned t = threadIdx.x;
+  unsigned v[4], sum = 0;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) { v[j] = hist[4 * t + j]; sum += v[j]; }
+  part[t] = sum;
+  __syncthreads();
+  for (unsigned off = 1; off < kOrderBins / 4; off <<= 1) {
+    unsigned add = t >= off ? part[t - off] : 0u;
+    __syncthreads();
+    part[t] += add;
+    __syncthreads();
+  }
+  unsigned run = part[t] - sum;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) { cursor[4 * t + j] = run; run += v[j]; }
+}
+
+__global__ void order_scatter_kernel(const int32_t *__restrict__ key, uint64_t n, const unsigned *kmax, unsigned *cursor,
+                                     int32_t *__restrict__ order) {
+  const unsigned km = *kmax;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
+    order[atomicAdd(&cursor[order_bin(key[i], km)], 1u)] = (int32_t)i;
 }
 
 __global__ void count_status_kernel(const int32_t *__restrict__ status, uint64_t n, gray2_stats *stats) {

@@ -35,7 +35,7 @@ class Gray2Error(RuntimeError):
 class _CState(C.Structure):
     _fields_ = [("q", C.c_void_p * 8), ("lam", C.c_void_p), ("status", C.c_void_p), ("nsteps", C.c_void_p),
                 ("n", C.c_uint64), ("a_eff", C.c_double), ("prec", C.c_int32), ("kind", C.c_int32),
-                ("reversed", C.c_int32), ("coords", C.c_int32)]
+                ("reversed", C.c_int32), ("coords", C.c_int32), ("order", C.c_void_p)]
 
 
 class StepControl(C.Structure):
@@ -84,6 +84,8 @@ def load_library():
     lib.gray2_convert.argtypes = [p, p, u64, i32, p]
     lib.gray2_flops_per_step_bl.argtypes = [i32]
     lib.gray2_set_launch.argtypes = [i32, i32, i32]
+    lib.gray2_order_longest_first.argtypes = [p, u64, p, p]
+    lib.gray2_order_longest_first.restype = C.c_int
     lib.gray2_flops_per_step.argtypes = [i32]
     for name in ("gray2_init_null", "gray2_init_timelike", "gray2_integrate", "gray2_invariants", "gray2_rhs",
                  "gray2_set_launch", "gray2_flops_per_step"):
@@ -124,6 +126,7 @@ class State:
     kind: int = NULL
     reversed: int = 0
     coords: int = KS
+    order: torch.Tensor | None = None     # optional (n,) int32 cuda: the schedule of the integrators (gray2.h)
 
     @staticmethod
     def empty(n: int, prec: int = F64, device="cuda") -> "State":
@@ -141,6 +144,9 @@ class State:
         s.lam, s.status, s.nsteps = self.lam.data_ptr(), self.status.data_ptr(), self.nsteps.data_ptr()
         s.n, s.a_eff, s.prec, s.kind, s.reversed = self.n, self.a_eff, self.prec, self.kind, self.reversed
         s.coords = self.coords
+        if self.order is not None:
+            assert self.order.is_cuda and self.order.dtype == torch.int32 and self.order.numel() == self.n
+            s.order = self.order.data_ptr()
         return s
 
     def _back(self, s: _CState):
@@ -148,7 +154,7 @@ class State:
 
     def clone(self) -> "State":
         return State(self.n, self.prec, self.q.clone(), self.lam.clone(), self.status.clone(),
-                     self.nsteps.clone(), self.a_eff, self.kind, self.reversed, self.coords)
+                     self.nsteps.clone(), self.a_eff, self.kind, self.reversed, self.coords, self.order)
 
 
 def init_null(a, r_obs, inclination_rad, fov_half_alpha, fov_half_beta, nx, ny, prec=F64, stream=None,
@@ -298,6 +304,17 @@ def convert(st: State, to_coords: int, n=None, stream=None, out: State | None = 
     _check(load_library().gray2_convert(C.byref(cs), C.byref(cd), n, to_coords, _stream_ptr(stream)))
     dst._back(cd)
     return dst
+
+
+def order_longest_first(steps_hint: torch.Tensor, stream=None, out: torch.Tensor | None = None) -> torch.Tensor:
+    """gray2_order_longest_first: the indices sorted by decreasing steps_hint (cuda int32), as a cuda int32 tensor
+    to put into State.order."""
+    assert steps_hint.is_cuda and steps_hint.dtype == torch.int32 and steps_hint.is_contiguous()
+    n = steps_hint.numel()
+    order = out if out is not None else torch.empty(n, dtype=torch.int32, device=steps_hint.device)
+    _check(load_library().gray2_order_longest_first(C.c_void_p(steps_hint.data_ptr()), n, C.c_void_p(order.data_ptr()),
+                                                    _stream_ptr(stream)))
+    return order
 
 
 def set_launch(prec, threads_per_block=0, blocks_per_sm=0):

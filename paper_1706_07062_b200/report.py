@@ -46,9 +46,17 @@ def run_image(cfg, prec):
     _, dt = _timed(lambda: gray2.integrate(st2, INF, sc, stats=stats))
     inv1 = gray2.invariants(st2)
     sd = gray2.stats_dict(stats)
+    # the same image once more, scheduled longest first with the step counts of the trace above as the hint
+    # (gray2_order_longest_first: what a caller that traces the same geometry repeatedly can do); same outputs
+    st3 = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec)
+    st3.order = gray2.order_longest_first(st2.nsteps)
+    _, dt_lf = _timed(lambda: gray2.integrate(st3, INF, sc))
+    identical = bool(torch.equal(st3.q, st2.q) and torch.equal(st3.nsteps, st2.nsteps))
+    del st3
     ns = st2.nsteps
     esc = st2.status == gray2.ESCAPED
     rep = dict(sd, rays=cfg.n, seconds=dt, steps_per_s=sd["steps"] / dt,
+               seconds_longest_first=dt_lf, steps_per_s_longest_first=sd["steps"] / dt_lf, longest_first_outputs_identical=identical,
                nsteps_min=int(ns.min()), nsteps_mean=float(ns.float().mean()), nsteps_max=int(ns.max()),
                captured_fraction=sd["n_captured"] / cfg.n,
                long_path_rays=int((ns > 1.5 * ns.float().mean()).sum()),
@@ -69,10 +77,7 @@ def spherical(q, a_eff):
     return r, th, ph
 
 
-def report_cfg3():
-    cfg = inputs.CFG3_NULL
-    s64, r64 = run_image(cfg, gray2.F64)
-    s32, r32 = run_image(cfg, gray2.F32)
+def compare_f32_f64(s64, s32, cfg):
     both_esc = (s64.status == gray2.ESCAPED) & (s32.status == gray2.ESCAPED)
     same = both_esc & (s64.nsteps == s32.nsteps)
     ra, ta, pa = spherical(s64.q, s64.a_eff)
@@ -92,12 +97,33 @@ def report_cfg3():
     cosang = (va * vb).sum(0) / (va.norm(dim=0) * vb.norm(dim=0))
     ang = torch.acos(torch.clamp(cosang, -1.0, 1.0))[both_esc]
     mask_diff = int(((s64.status == gray2.CAPTURED) != (s32.status == gray2.CAPTURED)).sum())
-    return {"f64": r64, "f32": r32,
-            "fp32_vs_fp64": {"escaped_in_both": int(both_esc.sum()), "equal_step_count_fraction": float(same.sum()) / max(int(both_esc.sum()), 1),
-                             "quantiles": [0.5, 0.9, 0.99, 0.999, 1.0],
-                             "final_r_relative": quant(err["r_rel"]), "final_theta_rad": quant(err["theta"]),
-                             "final_phi_rad": quant(err["phi"]), "velocity_direction_rad_all_escaped": quant(ang),
-                             "capture_mask_disagreements": mask_diff, "rays": cfg.n}}
+    return {"escaped_in_both": int(both_esc.sum()), "equal_step_count_fraction": float(same.sum()) / max(int(both_esc.sum()), 1),
+            "quantiles": [0.5, 0.9, 0.99, 0.999, 1.0],
+            "final_r_relative": quant(err["r_rel"]), "final_theta_rad": quant(err["theta"]),
+            "final_phi_rad": quant(err["phi"]), "velocity_direction_rad_all_escaped": quant(ang),
+            "rays_beyond_1e-4_in_r_theta_or_phi": int(((err["r_rel"] > 1e-4) | (err["theta"] > 1e-4) | (err["phi"] > 1e-4)).sum()),
+            "capture_mask_disagreements": mask_diff, "rays": cfg.n}
+
+
+def report_cfg3():
+    """BASELINE.json configs[2]: FP32-vs-FP64 error on the final (r, theta, phi) of escaped rays and on the capture
+    mask.  Twice: (i) each precision from its own gray2_init_null (the float image differs from the double one by
+    the rounding of the starting points, ~3e-5 M at r_obs = 1000 M), (ii) the double run started from the float
+    initial state, so that only the arithmetic of the integration differs."""
+    cfg = inputs.CFG3_NULL
+    s64, r64 = run_image(cfg, gray2.F64)
+    s32, r32 = run_image(cfg, gray2.F32)
+    out = {"f64": r64, "f32": r32, "fp32_vs_fp64": compare_f32_f64(s64, s32, cfg)}
+    del s64
+    i32 = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=gray2.F32)
+    w = gray2.State(i32.n, gray2.F64, i32.q.double(), i32.lam.clone(), i32.status.clone(), i32.nsteps.clone(),
+                    i32.a_eff, i32.kind, i32.reversed, i32.coords)
+    del i32
+    sc = gray2.step_control(mode=1, eta=cfg.eta, r_escape=cfg.r_escape, max_steps=cfg.max_steps,
+                            capture_factor=cfg.capture_factor)
+    gray2.integrate(w, INF, sc)
+    out["fp32_vs_fp64_same_float_inputs"] = compare_f32_f64(w, s32, cfg)
+    return out
 
 
 def report_cfg1():

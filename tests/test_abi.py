@@ -38,8 +38,8 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_struct_layouts_match_the_header(lib):
     from paper_1706_07062_b200 import gray2
-    # gray2_state: 8 pointers + 3 pointers + u64 + double + 3 int32 (+ pad) ; gray2_step_control per the header
-    assert C.sizeof(gray2._CState) == 8 * 8 + 3 * 8 + 8 + 8 + 16
+    # gray2_state: 8 pointers + 3 pointers + u64 + double + 4 int32 + the order pointer ; gray2_step_control per the header
+    assert C.sizeof(gray2._CState) == 8 * 8 + 3 * 8 + 8 + 8 + 16 + 8 and gray2._CState.order.offset == 120
     assert C.sizeof(gray2.StepControl) == 56
     assert gray2.StepControl.eta.offset == 16 and gray2.StepControl.max_steps.offset == 48
 
@@ -136,6 +136,9 @@ def test_new_entries_reject_bad_arguments_without_gpu_work(lib):
     assert lib.gray2_init_explicit(C.byref(s), 0.5, null, 16, 0, 0, null) == EINVAL   # no host array
     assert lib.gray2_init_explicit(C.byref(s), 0.5, fake, 17, 0, 0, null) == ESTATE   # n > s->n
     assert lib.gray2_init_explicit(C.byref(s), 1.5, fake, 16, 1, 0, null) == EINVAL   # |a| > 1
+    assert lib.gray2_order_longest_first(null, 16, fake, null) == EINVAL              # no hint array
+    assert lib.gray2_order_longest_first(fake, 0, fake, null) == EINVAL               # n == 0
+    assert lib.gray2_order_longest_first(fake, 1 << 31, fake, null) == EINVAL         # indices are int32
     assert not hasattr(lib, "gray2_fma_probe")        # the probe kernels live in bench_probe.cu, not in the product
 
 

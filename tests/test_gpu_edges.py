@@ -181,6 +181,45 @@ def test_more_calls_in_flight_than_work_queue_slots():
         assert gray2.stats_dict(st) == ref_stats
 
 
+def test_schedule_changes_no_output_bit():
+    """gray2_state.order (optional order array): the longest-first order from a previous
+    trace is a permutation sorted by decreasing step count, and integrating with it -- in both precisions, in
+    the coordinate-time and Boyer-Lindquist forms -- gives the outputs of the unordered run bit for bit."""
+    cfg = inputs.CFG3_NULL.scaled(160, 123)
+    gsc, _ = image_sc(cfg)
+    for prec in (gray2.F64, gray2.F32):
+        for form in ("affine", "coordtime", "bl"):
+            def fresh():
+                g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec)
+                return gray2.convert(g, gray2.BL) if form == "bl" else g
+            run = gray2.integrate_coordtime if form == "coordtime" else gray2.integrate
+            ref, sref = fresh(), gray2.new_stats()
+            run(ref, INF, gsc, stats=sref)
+            order = gray2.order_longest_first(ref.nsteps)
+            o = order.cpu().numpy()
+            assert np.array_equal(np.sort(o), np.arange(cfg.n))
+            hint = ref.nsteps.cpu().numpy()[o].astype(np.int64)
+            width = int(hint.max()) // 4096 + 1               # 4096 bins over [0, max]: sorted up to the bin width
+            assert (np.diff((hint.max() - hint) // width) >= 0).all() and hint.max() - hint[0] < width
+            g, sg = fresh(), gray2.new_stats()
+            g.order = order
+            run(g, INF, gsc, stats=sg)
+            torch.cuda.synchronize()
+            assert torch.equal(ref.q, g.q) and torch.equal(ref.nsteps, g.nsteps) and torch.equal(ref.status, g.status)
+            assert torch.equal(ref.lam, g.lam) and torch.equal(sref, sg)
+    # a call that covers only part of the state ignores the schedule (it would not be a permutation of that part)
+    a = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    b = a.clone()
+    b.order = order
+    gray2.integrate(a, INF, gsc, n=1000)
+    gray2.integrate(b, INF, gsc, n=1000)
+    assert torch.equal(a.q, b.q) and torch.equal(a.status, b.status) and (b.status[1000:] == gray2.ACTIVE).all()
+    # hints with a huge range (bins wider than one), zeros and negatives
+    hint = torch.tensor([5, 0, -3, 2_000_000_000, 17, 17, 1_000_000], dtype=torch.int32, device="cuda")
+    o = gray2.order_longest_first(hint).cpu().numpy()
+    assert sorted(o.tolist()) == list(range(7)) and o[0] == 3 and o[1] == 6
+
+
 def test_fma_probes_of_the_bench_run_in_every_form():
     """The FMA-only kernels behind bench.py's fma_probe_* fields live in bench_probe.cu (not in the product
     library): every operand form launches, bad forms are refused."""
