@@ -495,6 +495,10 @@ def block_of(job: Job, m: dict, t_step, t_int, steps_all, t_e2e, e2e_all) -> dic
                      "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/kernel_counters.csv)",
                      "algorithmic_bytes": 2 * (80 if dtype == "f64" else 48) * job.n_local,
                      "flops_per_rk4_step": fps,
+                     # FP32 only: the same fraction with the count of the uncompensated step (round 1's: 530 affine,
+                     # 534 coordinate time, 566 Boyer-Lindquist), i.e. without the 3 additions per state variable
+                     "frac_without_compensation_flops": (achieved / peak) * (fps - (18 if job.coord else 24)) / fps
+                                                        if dtype == "f32" else None,
                      "kernel_ms": 1e3 * t_int / args.steps, "kernel_ms_best": 1e3 * best_int,
                      "kernel_share_of_step": t_int / t_step,
                      "peak_source": "nominal: %d SMs x %d lanes x 2 x %.0f MHz" % (job.n_sms, FP_LANES[dtype], job.sm_max_mhz),

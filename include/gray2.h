@@ -228,7 +228,8 @@ int gray2_order_longest_first(const int32_t *steps_hint, uint64_t n, int32_t *or
 int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm);
 
 /* Exact floating-point operation counts of one RK4 step of one geodesic in this library's code path
- * (FMA = 2 flops, add/mul = 1, each rsqrt/rcp = 1), used for the roofline figure; see DESIGN.md. */
+ * (FMA = 2 flops, add/mul = 1, each rsqrt/rcp = 1), used for the roofline figure; see DESIGN.md.  The FP32
+ * counts include the three extra additions per state variable of the compensated sums (530 + 24 = 554). */
 int gray2_flops_per_step(int32_t prec);
 int gray2_flops_per_step_coordtime(int32_t prec);
 int gray2_flops_per_step_bl(int32_t prec);

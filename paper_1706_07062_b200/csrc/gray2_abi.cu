@@ -98,6 +98,7 @@ template <typename T> gray2::StateView<T> view_of(const gray2_state *s) {
   gray2::StateView<T> v;
   for (int m = 0; m < 8; ++m) v.q[m] = static_cast<T *>(s->q[m]);
   v.lambda = s->lambda; v.status = s->status; v.nsteps = s->nsteps;
+  v.order = s->order;
   return v;
 }
 
@@ -117,39 +118,37 @@ int check_state(const gray2_state *s, const char *who) {
 // ---- integrator dispatch ----------------------------------------------------------------------------
 namespace {
 
-template <typename T, int THREADS, int MIN_BLOCKS, int FORM>
+template <typename T, int THREADS, int MIN_BLOCKS, int FORM, bool ORDERED = false>
 cudaError_t launch_integrate(const gray2_state *s, uint64_t n, const gray2::StepParams<T> &p,
                              unsigned long long *queue, unsigned long long *steps, int num_sms, cudaStream_t st) {
   uint64_t want = (n + THREADS - 1) / THREADS;
   uint64_t cap = (uint64_t)num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<T>(s);
-  const int32_t *order = n == s->n ? s->order : nullptr;      // a schedule covers the whole state or is not used
   if (p.mode == 1) {
-    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
-    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, true, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 1, false, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
   } else {
-    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
-    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    if (p.clip) gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, true, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel<T, THREADS, MIN_BLOCKS, 0, false, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
   }
   return cudaGetLastError();
 }
 
 // FP32 with two geodesics per thread (packed FP32x2 arithmetic)
-template <int THREADS, int MIN_BLOCKS, int FORM>
+template <int THREADS, int MIN_BLOCKS, int FORM, bool ORDERED = false>
 cudaError_t launch_integrate_x2(const gray2_state *s, uint64_t n, const gray2::StepParams<float> &p,
                                 unsigned long long *queue, unsigned long long *steps, int num_sms, cudaStream_t st) {
   uint64_t want = (n + 2 * THREADS - 1) / (2 * THREADS);
   uint64_t cap = (uint64_t)num_sms * MIN_BLOCKS;
   unsigned grid = (unsigned)(want < cap ? want : cap);
   auto v = view_of<float>(s);
-  const int32_t *order = n == s->n ? s->order : nullptr;
   if (p.mode == 1) {
-    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
-    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, true, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 1, false, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
   } else {
-    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, true, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
-    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, false, FORM><<<grid, THREADS, 0, st>>>(v, n, p, order, queue, steps);
+    if (p.clip) gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, true, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
+    else        gray2::integrate_kernel_f32x2<THREADS, MIN_BLOCKS, 0, false, FORM, ORDERED><<<grid, THREADS, 0, st>>>(v, n, p, queue, steps);
   }
   return cudaGetLastError();
 }
@@ -170,6 +169,19 @@ cudaError_t dispatch_integrate(int form, int threads, int blocks, const gray2_st
                                const gray2::StepParams<T> &p, unsigned long long *q, unsigned long long *steps,
                                int sms, cudaStream_t st, bool *found) {
   *found = true;
+  // A schedule (gray2_state.order) is used only by a call that covers the whole state, and runs in the default
+  // launch shape of its form (the ordered kernels are compiled for that shape only).
+  if (s->order && n == s->n) {
+    if constexpr (sizeof(T) == 8) {
+      if (form == 1) return launch_integrate<T, 128, 3, 1, true>(s, n, p, q, steps, sms, st);
+      if (form == 2) return launch_integrate<T, 128, 3, 2, true>(s, n, p, q, steps, sms, st);
+      return launch_integrate<T, 128, 3, 0, true>(s, n, p, q, steps, sms, st);
+    } else {
+      if (form == 1) return launch_integrate_x2<256, 2, 1, true>(s, n, p, q, steps, sms, st);
+      if (form == 2) return launch_integrate_x2<256, 2, 2, true>(s, n, p, q, steps, sms, st);
+      return launch_integrate_x2<256, 2, 0, true>(s, n, p, q, steps, sms, st);
+    }
+  }
   if constexpr (sizeof(T) == 8) {
     if (form == 1) return launch_integrate<T, 128, 3, 1>(s, n, p, q, steps, sms, st);
     if (form == 2) {
@@ -560,18 +572,22 @@ int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void
 
 /* Source-level count of ks_geodesic.cuh (FMA = 2, add/mul = 1, rsqrt/rcp = 1; negations and compares free):
  *   radius 16, rest of geometry 19, velocity part 72  ->  107 per right-hand side
- *   4 x 107 + RK4 combination 100 + step rule and lambda update 2 = 530 per step (both precisions). */
-int gray2_flops_per_step(int32_t prec) { (void)prec; return 530; }
+ *   4 x 107 + RK4 combination 100 + step rule and lambda update 2 = 530 per step in double.
+ * FP32 carries the eight state sums compensated (Carry<T>, ks_geodesic.cuh): each y <- y + w S costs an FMA and
+ * three additions instead of one FMA, + 3 per variable = + 24 per step: 554. */
+int gray2_flops_per_step(int32_t prec) { return prec == GRAY2_F32 ? 554 : 530; }
 
-/* Coordinate-time form: 4 x (107 + 6) + RK4 combination of six variables 80 + step rule and t update 2. */
-int gray2_flops_per_step_coordtime(int32_t prec) { (void)prec; return 534; }
+/* Coordinate-time form: 4 x (107 + 6) + RK4 combination of six variables 80 + step rule and t update 2 = 534;
+ * FP32: six compensated sums, + 18. */
+int gray2_flops_per_step_coordtime(int32_t prec) { return prec == GRAY2_F32 ? 552 : 534; }
 
 /* Boyer-Lindquist form, source-level count of bl_geodesic.cuh (same conventions):
  *   sin^2 and sin cos of theta: reduction 8, series 17 + 16, products 2 -> 43 (double: 8 / 8 terms, period pi/2),
  *                               reduction 8, series 13 + 12, products 2 -> 35 (float: 6 / 6 terms, period pi)
  *   rest of the right-hand side 81 (4 of them reciprocals)  ->  124 / 116 per right-hand side
- *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 598 / 566 per step. */
-int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 566 : 598; }
+ *   4 x RHS + RK4 combination 94 + finiteness probe 6 + step rule and lambda update 2 = 598 / 566 per step;
+ *   FP32: eight compensated sums, + 24 = 590. */
+int gray2_flops_per_step_bl(int32_t prec) { return prec == GRAY2_F32 ? 590 : 598; }
 
 int gray2_order_longest_first(const int32_t *steps_hint, uint64_t n, int32_t *order, void *cuda_stream) {
   if (!steps_hint || !order || n == 0) return fail(GRAY2_EINVAL, "gray2_order_longest_first: NULL pointer or n == 0");

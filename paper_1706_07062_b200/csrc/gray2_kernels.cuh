@@ -22,6 +22,7 @@ template <typename T> struct StateView {
   double *lambda;
   int32_t *status;
   int32_t *nsteps;
+  const int32_t *order;     // gray2_state.order; read by the ORDERED instantiations of the integrators only
 };
 
 template <typename T> struct StepParams {
@@ -103,10 +104,13 @@ __global__ void init_explicit_kernel(StateView<T> s, const double *__restrict__ 
 // clock `lam` is then t itself, v^i = u^i/u^t on load, and (t, x, 1, v) is stored; `lambda` is untouched;
 // 2 affine parameter in Boyer-Lindquist coordinates (bl_geodesic.cuh): the state is (t, r, theta, phi) and
 // its derivatives, the radius of the step rule and of the stopping tests is the coordinate r itself.
-template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
+//
+// ORDERED: the queue position is mapped to a geodesic through the caller's schedule s.order (gray2_state.order);
+// a separate instantiation, so that the code of the unordered kernel does not depend on the feature.
+template <typename T, int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM, bool ORDERED = false>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
-integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, const int32_t *__restrict__ order,
-                 unsigned long long *queue, unsigned long long *steps_out) {
+integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long *queue,
+                 unsigned long long *steps_out) {
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
   const SpinConst<T> k = p.k;
@@ -138,7 +142,7 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, const int32_t *__r
       if (!have) {
         uint64_t mine = base + __popc(idle & lt_mask);      // position in the queue
         if (mine < n) {
-          if (order) mine = (uint64_t)order[mine];          // ... and the geodesic the caller's schedule puts there
+          if constexpr (ORDERED) mine = (uint64_t)s.order[mine];   // ... and the geodesic the schedule puts there
           // the status and the state are fetched together (one round trip to memory instead of two); an entry
           // that turns out not to be ACTIVE is dropped and its slot of the lane refilled at the next pass
           const int32_t st_in = s.status[mine];
@@ -245,11 +249,11 @@ struct PairSlot {
   bool cap;     // FORM 2: the last step was rejected, a stage reached the capture radius
 };
 
-template <int C, int FORM>
-__device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, const int32_t *__restrict__ order,
-                                          uint64_t mine, Ray<f32x2> &ray, Carry<f32x2> &car, PairSlot &sl) {
+template <int C, int FORM, bool ORDERED>
+__device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, uint64_t mine, Ray<f32x2> &ray,
+                                          Carry<f32x2> &car, PairSlot &sl) {
   if (mine >= n) return;
-  if (order) mine = (uint64_t)order[mine];
+  if constexpr (ORDERED) mine = (uint64_t)s.order[mine];
   // the status and the state are fetched together (one round trip to memory instead of two)
   const int32_t st_in = s.status[mine];
   float t = s.q[0][mine], x = s.q[1][mine], y = s.q[2][mine], z = s.q[3][mine];
@@ -307,10 +311,10 @@ __device__ __forceinline__ void store_slot(const StateView<float> &s, const Step
   sl.have = false;
 }
 
-template <int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM>
+template <int THREADS, int MIN_BLOCKS, int MODE, bool CLIP, int FORM, bool ORDERED = false>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
-integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, const int32_t *__restrict__ order,
-                       unsigned long long *queue, unsigned long long *steps_out) {
+integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, unsigned long long *queue,
+                       unsigned long long *steps_out) {
   const unsigned lane = threadIdx.x & 31u;
   const unsigned lt_mask = (1u << lane) - 1u;
   const SpinConst<f32x2> k{f32x2(p.k.a), f32x2(p.k.a2), f32x2(p.k.two_a), f32x2(p.k.two_a2), f32x2(p.k.four_a2)};
@@ -333,8 +337,8 @@ integrate_kernel_f32x2(StateView<float> s, uint64_t n, StepParams<float> p, cons
       if (lane == 0) base = atomicAdd(queue, (unsigned long long)cnt);
       base = __shfl_sync(0xffffffffu, base, 0);
       if (base + cnt >= n) drained = true;
-      if (!A.have) load_slot<0, FORM>(s, n, order, base + __popc(idleA & lt_mask), ray, car, A);
-      if (!B.have) load_slot<1, FORM>(s, n, order, base + cntA + __popc(idleB & lt_mask), ray, car, B);
+      if (!A.have) load_slot<0, FORM, ORDERED>(s, n, base + __popc(idleA & lt_mask), ray, car, A);
+      if (!B.have) load_slot<1, FORM, ORDERED>(s, n, base + cntA + __popc(idleB & lt_mask), ray, car, B);
       continue;
     }
     if ((idleA & idleB) == 0xffffffffu) break;

@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol(lib):
     for name in declared_functions():
         assert hasattr(lib, name), name
     assert b"sm_100a" in lib.gray2_version()
-    assert lib.gray2_flops_per_step(0) == 530 and lib.gray2_flops_per_step(1) == 530
+    assert lib.gray2_flops_per_step(0) == 530 and lib.gray2_flops_per_step(1) == 554
 
 
 def test_struct_layouts_match_the_header(lib):
@@ -127,8 +127,8 @@ def test_new_entries_reject_bad_arguments_without_gpu_work(lib):
     s.n = 15
     assert lib.gray2_init_null_shard(C.byref(s), *args, 8, 0, 2, null) == EINVAL      # shard has 16 rays, state 15
     assert lib.gray2_rhs_bl(0, 0.5, 0, null, null, null, null) == EINVAL
-    assert lib.gray2_flops_per_step_bl(0) == 598 and lib.gray2_flops_per_step_bl(1) == 566
-    assert lib.gray2_flops_per_step_coordtime(0) == 534
+    assert lib.gray2_flops_per_step_bl(0) == 598 and lib.gray2_flops_per_step_bl(1) == 590
+    assert lib.gray2_flops_per_step_coordtime(0) == 534 and lib.gray2_flops_per_step_coordtime(1) == 552
     fake = C.c_void_p(0x1000)
     s.n = 16
     assert lib.gray2_init_explicit(C.byref(s), 0.5, fake, 16, 7, 0, null) == EINVAL   # unknown kind
