@@ -250,6 +250,12 @@ int integrate_impl(int form, gray2_state *s, uint64_t n, double end, const gray2
   const uint32_t chosen = g_launch[pi].load(std::memory_order_relaxed);
   int threads = chosen ? (int)(chosen >> 16) : def.threads;
   int blocks = chosen ? (int)(chosen & 0xffffu) : def.blocks;
+  // Small batches: a geodesic is ~1000 sequential steps, so a batch that cannot fill the GPU is bound by the
+  // latency of one step, and what matters is to spread it over the SMs.  The packed FP32 kernel (512 geodesics per
+  // block) would put cfg1's 4,096 rays on 8 SMs; the one-per-thread float kernel (128 per block) gives the same
+  // bits from 32.  Only the affine Kerr-Schild form has that variant compiled, and only an unset launch choice
+  // is overridden.
+  if (sizeof(T) == 4 && !chosen && form == 0 && n < (uint64_t)qs.num_sms * 512) { threads = 128; blocks = 8; }
   bool found = false;
   cudaError_t e = dispatch_integrate<T>(form, threads, blocks, s, n, p, queue, steps, qs.num_sms, st, &found);
   if (!found) return fail(GRAY2_EINVAL, "gray2_integrate: no compiled variant for %d threads x %d blocks/SM", threads, blocks);
