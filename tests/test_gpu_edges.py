@@ -181,6 +181,48 @@ def test_more_calls_in_flight_than_work_queue_slots():
         assert gray2.stats_dict(st) == ref_stats
 
 
+def test_set_launch_may_race_with_integrations():
+    """gray2.h: any number of host threads may call in.  One thread keeps switching the launch shape among the
+    compiled variants while four others integrate: no call may fail ("no compiled variant" would be a torn read
+    of the pair) and every result equals the reference bit for bit."""
+    import threading
+    cfg = inputs.CFG3_NULL.scaled(96, 64)
+    gsc, _ = image_sc(cfg)
+    ref = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny)
+    gray2.integrate(ref, INF, gsc)
+    torch.cuda.synchronize()
+    stop, errors = threading.Event(), []
+
+    def switcher():
+        shapes = [(128, 3), (128, 4), (64, 6), (256, 1), (128, 2), (0, 0)]
+        k = 0
+        while not stop.is_set():
+            gray2.set_launch(gray2.F64, *shapes[k % len(shapes)])
+            k += 1
+
+    def worker():
+        try:
+            stream = torch.cuda.Stream()
+            for _ in range(12):
+                with torch.cuda.stream(stream):
+                    g = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, stream=stream)
+                    gray2.integrate(g, INF, gsc, stream=stream)
+                stream.synchronize()
+                assert torch.equal(g.q, ref.q) and torch.equal(g.nsteps, ref.nsteps) and torch.equal(g.status, ref.status)
+        except Exception as exc:          # noqa: BLE001
+            errors.append(exc)
+
+    sw = threading.Thread(target=switcher)
+    sw.start()
+    ws = [threading.Thread(target=worker) for _ in range(4)]
+    for w in ws: w.start()
+    for w in ws: w.join()
+    stop.set()
+    sw.join()
+    gray2.set_launch(gray2.F64, 0, 0)
+    assert not errors, errors
+
+
 def test_schedule_changes_no_output_bit():
     """gray2_state.order (optional order array): the longest-first order from a previous
     trace is a permutation sorted by decreasing step count, and integrating with it -- in both precisions, in

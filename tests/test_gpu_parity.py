@@ -66,6 +66,35 @@ def test_init_timelike_matches_oracle():
         assert np.max(np.abs(a_ - b_) / np.maximum(np.abs(b_), 1.0)) < 1e-13
 
 
+def test_init_explicit_of_either_kind_matches_oracle(table1):
+    """The paper's Table 1 orbits are explicit PHOTON data: through gray2_init_explicit with
+    kind = NULL the state-level invariants are (1, Phi, Q, 0) with no patching of the struct; the kind decides
+    mu^2 in Carter's Q and in the u^t solve, exactly as in the oracle."""
+    import closed_forms as cf
+    xu8 = np.array([cf.spherical_photon_state(1.0, r["r"])[0] for r in table1])
+    moved = np.array([oracle.trajectory(1.0, y, 1.0 / 64, 40)[-1] for y in xu8])     # off the equator: mu^2 enters Q
+    for kind in (gray2.NULL, gray2.TIMELIKE):
+        for data in (xu8, moved):
+            for renorm in (False, True):
+                x = data.copy()
+                if renorm:
+                    x = x[[0, 2, 3, 4, 5]]            # rows B's start (r = 2, a = 1) is on the ergosphere: 1 - f = 0
+                    x[:, 4] = 99.0
+                g = gray2.init_explicit(1.0, x, kind, renormalise_ut=renorm)
+                o = oracle.init_explicit(1.0, x, kind, renormalise_ut=renorm)
+                assert (g.kind, g.reversed, g.a_eff) == (kind, 0, 1.0) == (o.kind, o.reversed, o.a_eff)
+                assert np.max(np.abs(g.q.cpu().numpy() - o.q) / np.maximum(np.abs(o.q), 1.0)) < 1e-13
+                for a_, b_ in zip(gpu_invariants_np(g), oracle.invariants(o)):
+                    assert np.max(np.abs(a_ - b_) / np.maximum(np.abs(b_), 1.0)) < 1e-12
+    E, Lz, Q, norm = gpu_invariants_np(gray2.init_explicit(1.0, xu8, gray2.NULL))
+    for k, row in enumerate(table1):
+        assert abs(E[k] - 1) < 1e-13 and abs(Lz[k] - row["phi"]) < 5e-5 and abs(Q[k] - row["q"]) < 5e-5 and abs(norm[k]) < 1e-13
+    with pytest.raises(gray2.Gray2Error):
+        gray2.init_explicit(1.0, xu8, 7)
+    t = gray2.init_timelike(1.0, xu8)
+    assert t.kind == gray2.TIMELIKE and torch.equal(t.q, gray2.init_explicit(1.0, xu8, gray2.TIMELIKE).q)
+
+
 # ---- whole path on image configs ------------------------------------------------------------------
 
 def compare_image(cfg, g0, g, o0, o, idx=None):
