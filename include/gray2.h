@@ -7,7 +7,8 @@
  *
  * What is computed (all of it in CUDA kernels for sm_100a; there is no CPU fallback):
  *   gray2_init_null      image-plane initial conditions of null geodesics      PAPER.md:296; DESIGN R1-R3
- *   gray2_init_timelike  explicit 8-vectors (t,x,y,z,u^t,u^x,u^y,u^z)
+ *   gray2_init_explicit  explicit 8-vectors (t,x,y,z,u^t,u^x,u^y,u^z) of photons or particles
+ *   (gray2_init_timelike: its time-like case)
  *   gray2_integrate      classic RK4 of the geodesic equation in Cartesian Kerr-Schild
  *                        coordinates, metric g = eta + f l l (eq. 2-5), right-hand side in
  *                        the regrouped form of eq. (10)-(14), each geodesic advanced
@@ -17,13 +18,15 @@
  * and, around these four: gray2_integrate_coordtime (the coordinate-time form),
  * gray2_integrate_diagnostics (the convergence measurements of section 3), gray2_convert plus
  * gray2_state.coords (the Boyer-Lindquist system of the paper's Table 2, behind the same gray2_integrate),
- * gray2_init_null_shard (one image shared by several GPUs).
+ * gray2_init_null_shard (one image shared by several GPUs), gray2_state.order plus
+ * gray2_order_longest_first (an optional schedule of the integrators).
  *
  * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
  * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
  * library allocates no device memory of its own except a 4 KiB work-queue scratch per device (64 slots
  * handed out round-robin; a call that gets a slot whose previous user is still running waits for it on
- * the device, so any number of integrations may be in flight) and the staging buffers
+ * the device, so any number of integrations may be in flight), the 32 KiB histogram of
+ * gray2_order_longest_first (per device, allocated at its first call) and the staging buffers
  * of gray2_init_explicit (per device; n x 64 bytes each, one per calling stream up to eight, grown on demand,
  * reused, released at process exit).  `host_xu8` is a HOST pointer.
  * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
