@@ -126,6 +126,13 @@ def compare_image(cfg, g0, g, o0, o, idx=None):
     scales = [np.maximum(s1, s0) for s1, s0 in zip(invariant_term_scales(o.q), invariant_term_scales(o0.q))]
     for k, (gd, od) in enumerate(zip(drift(gi1, gi0), drift(oi1, oi0))):
         scale = scales[k]
+        # beside the term-scaled figure, the plain one: the difference of the two drifts relative to the drift itself
+        # (rms over the rays) and the largest difference relative to max(1, |invariant|)
+        rms_d = np.sqrt(np.mean(od[same] ** 2))
+        print("[drift %s] %-3s rms drift %.2e; GPU - oracle: rms %.2e (%.1e of the drift), max %.2e of max(1,|value|), max %.2e of the terms"
+              % (cfg.name, ("E", "Lz", "Q", "u.u")[k], rms_d, np.sqrt(np.mean((gd - od)[same] ** 2)),
+                 np.sqrt(np.mean((gd - od)[same] ** 2)) / max(rms_d, 1e-300),
+                 np.max(np.abs(gd - od)[same] / np.maximum(1.0, np.abs(oi0[k][same]))), np.max(np.abs(gd - od)[same] / scale[same])))
         assert np.max(np.abs(gd - od)[same] / scale[same]) < TOL_DRIFT_F64, (k, np.max(np.abs(gd - od)[same] / scale[same]))
     return outside, same
 
