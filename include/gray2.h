@@ -186,7 +186,9 @@ int gray2_convert(const gray2_state *src, gray2_state *dst, uint64_t n, int32_t 
  * reaches t_end stays ACTIVE ("integrate to a target KS coordinate time", method i).
  * On entry v^i = q[5+i] / q[4]; on exit q[0] = t, q[4] = 1 and q[5..7] = v^i (DESIGN R19): a tangent
  * vector of the same curve with another normalisation, so ratios such as L_z/E and Q/E^2 from
- * gray2_invariants keep their meaning.  s->lambda is not touched.  device_stats as for gray2_integrate. */
+ * gray2_invariants keep their meaning.  s->lambda is not touched.  device_stats as for gray2_integrate.
+ * FP32 states: the clock is q[0], a float, so t_end is rounded to float too: a geodesic that has reached the target
+ * holds exactly float(t_end), and a second identical call is a no-op as in double. */
 int gray2_integrate_coordtime(gray2_state *s, uint64_t n, double t_end, const gray2_step_control *sc,
                               int32_t prec, gray2_stats *device_stats, void *cuda_stream);
 

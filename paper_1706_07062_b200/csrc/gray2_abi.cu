@@ -237,6 +237,10 @@ gray2::StepParams<T> make_params(double a, double end, const gray2_step_control 
 template <typename T>
 int integrate_impl(int form, gray2_state *s, uint64_t n, double end, const gray2_step_control *sc,
                    gray2_stats *device_stats, cudaStream_t st) {
+  // Coordinate-time form in FP32: the clock is q[0] itself, a float.  The target is rounded to float as well, so that
+  // a geodesic that has reached it holds exactly the target and a second identical call is a no-op (with the double
+  // target a stored float(t_end) < t_end would ask for one more, rounding-sized, step at every call).
+  if (form == 1 && sizeof(T) == 4 && isfinite(end)) end = (double)(float)end;
   const gray2::StepParams<T> p = make_params<T>(s->a_eff, end, sc, /*always_clip=*/false);
 
   QueueSlot qs;

@@ -293,6 +293,33 @@ def test_backward_direction_and_lambda_clip():
     assert np.max(np.abs(back.q - xu8.T)) < 1e-6     # retraces the segment to truncation error
 
 
+@pytest.mark.parametrize("prec", [gray2.F64, gray2.F32], ids=["f64", "f32"])
+def test_clipped_step_lands_on_the_end_value_exactly(prec):
+    """DESIGN R22 on the GPU, all integrators: after a clipped last step the clock IS lambda_end (t_end), also where
+    lambda + (lambda_end - lambda) != lambda_end in double (0.03 -> 0.283 overshoots, 0.05 -> 0.216 falls short), and
+    the step counts equal the oracle's; a second identical call does nothing."""
+    xu8, _ = inputs.cfg4_ensemble(100)
+    for first, second in ((0.03, 0.283), (0.05, 0.216)):
+        for name, grun, orun in (("affine", gray2.integrate, oracle.integrate),
+                                 ("coordtime", gray2.integrate_coordtime, oracle.integrate_coordtime),
+                                 ("diagnostics", lambda *a, **k: gray2.integrate_diagnostics(*a, **k) and k.get("stats"),
+                                  lambda *a: oracle.integrate_diagnostics(*a)[0])):
+            g = gray2.init_timelike(0.7, xu8, prec=prec)
+            o = oracle.init_timelike(0.7, xu8)
+            gsc, osc = sc_pair(mode=0, h_fixed=1.0, max_steps=10 ** 6)
+            stats = gray2.new_stats()
+            for end in (first, second, second):
+                grun(g, end, gsc, stats=stats)
+                ostats = orun(o, end, osc)
+                torch.cuda.synchronize()
+                assert gray2.stats_dict(stats) == ostats, (name, end)
+                clock = g.q[0].double() if name == "coordtime" else g.lam
+                # (the coordinate-time clock is q[0] itself: a float in FP32 states, so the end value as a float)
+                expect = float(np.float32(end)) if (name == "coordtime" and prec == gray2.F32) else end
+                assert bool((clock == expect).all()), (name, end, clock[:3])
+            assert ostats["steps"] == 0 and bool((g.nsteps == 2).all())
+
+
 # ---- full-size configs, in the launch configuration bench.py times, against sampled oracle rays -----
 
 @pytest.mark.parametrize("cfg,nsample", [(inputs.CFG3_NULL, 1536), (inputs.CFG2_NULL, 1024)], ids=lambda c: getattr(c, "name", str(c)))
