@@ -63,6 +63,12 @@ def test_same_final_state_as_gray2_integrate():
     assert torch.equal(a_.q, b_.q) and torch.equal(a_.nsteps, b_.nsteps) and torch.equal(a_.status, b_.status)
     assert torch.equal(a_.lam, b_.lam)
     assert torch.isfinite(d["max_abs_u2"]).all() and (d["max_abs_u2"] < 1e-3).all() and d["max_abs_u2"].median() < 1e-9
+    # FP32: the diagnostics kernel carries the same compensated sums as the integrators (packed and scalar)
+    a32 = gray2.init_timelike(0.7, xu8, prec=gray2.F32)
+    b32 = gray2.init_timelike(0.7, xu8, prec=gray2.F32)
+    gray2.integrate(a32, INF, gsc)
+    gray2.integrate_diagnostics(b32, INF, gsc)
+    assert torch.equal(a32.q, b32.q) and torch.equal(a32.nsteps, b32.nsteps) and torch.equal(a32.lam, b32.lam)
 
 
 def test_epicyclic_frequency_batch_on_gpu():
