@@ -194,3 +194,37 @@ def test_bench_probe_object_builds_and_is_separate_from_the_product():
     assert lib.bench_fma_probe(0, 3, 1, 32, 1, C.c_void_p(0x1000), None) == 1        # packed form is FP32 only
     assert lib.bench_fma_probe(1, 2, 1, 32, 1, None, None) == 1                      # no scratch
     assert bench.load_counters("cfg3", "f64", "affine") is not None
+
+
+def test_bench_line_blocks_are_assembled_from_the_measurements():
+    """bench.block_of (the JSON fields of one precision) from synthetic per-rank measurements: no GPU needed.
+    Checks the arithmetic of value / roofline / executed_frac / e2e and that the profiler-only figures come from
+    profiles/kernel_counters.csv."""
+    import types
+    import bench
+    F64, F32 = 0, 1
+    flops = {F64: 530, F32: 554}
+    gray2 = types.SimpleNamespace(F64=F64, F32=F32)
+    args = types.SimpleNamespace(steps=2, workload="cfg3", form="affine")
+    job = types.SimpleNamespace(args=args, cfg=None, gray2=gray2, n_sms=148, sm_max_mhz=1965.0, world=1, strong=False,
+                                coord=False, bl=False, n_local=1 << 20, flops_per_step=lambda prec: flops[prec])
+    for dtype, prec in (("f64", F64), ("f32", F32)):
+        m = dict(dtype=dtype, prec=prec, per_step=[0.030, 0.028], per_int=[0.0295, 0.0275], steps_total=2_200_000_000,
+                 clocks={"sm_mhz": 1965.0, "reasons": []}, h2d=64, d2h=80, n_chunks=32, n_streams=8,
+                 probe={"imm": 36.0, "regs": 34.0, "fresh": 24.6, "packed": 48.7}, warmup=3)
+        b = bench.block_of(job, m, t_step=0.058, t_int=0.057, steps_all=2.2e9, t_e2e=0.06, e2e_all=2.2e9)
+        peak = 148 * (64 if dtype == "f64" else 128) * 2 * 1965e6 / 1e12
+        assert abs(b["value"] - 2.2e9 / 0.058) < 1 and abs(b["ms_per_step"] - 29.0) < 1e-9
+        assert abs(b["ms_per_step_best"] - 28.0) < 1e-9 and abs(b["ms_per_step_median"] - 29.0) < 1e-9
+        r = b["roofline"]
+        assert abs(r["peak"] - peak) < 1e-9 and r["bound"] == "alu" and r["unit"] == "TFLOP/s"
+        assert abs(r["achieved"] - 2.2e9 * flops[prec] / 0.057 / 1e12) < 1e-9 and abs(r["frac"] - r["achieved"] / peak) < 1e-12
+        row = bench.load_counters("cfg3", dtype, "affine")
+        assert r["traffic"] == int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+        assert abs(r["executed_frac"] - 2.2e9 * float(row["executed_flops_per_step"]) / 0.057 / 1e12 / peak) < 1e-12
+        assert r["algorithmic_bytes"] == 2 * (80 if dtype == "f64" else 48) * (1 << 20)
+        assert b["e2e"]["h2d_bytes_per_step"] == 64 and abs(b["e2e"]["value"] - 2.2e9 / 0.06) < 1
+        assert b["gpu_launches"] == 8
+        if dtype == "f32":
+            assert abs(r["frac_without_compensation_flops"] - r["frac"] * 530 / 554) < 1e-12
+    assert bench.load_counters("cfg9", "f64", "affine") is None
