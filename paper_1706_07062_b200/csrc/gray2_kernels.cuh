@@ -155,15 +155,25 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
           if (st_in == GRAY2_ACTIVE) {
             idx = mine;
             ray = in;
+            car.clear();
             if constexpr (FORM == 1) {
               lam = (double)ray.t;
-              T w = fastmath<T>::rcp(ray.u0);
-              ray.u1 *= w; ray.u2 *= w; ray.u3 *= w; ray.u0 = T(1);
+              if constexpr (Carry<T>::compensated) {
+                // FP32: v = u / u^t in double, split into the float the right-hand side sees and the residual of
+                // the compensated sum, so that the coordinate velocity starts without a rounding error of its own
+                // (a float division here is 1.5 ulp of direction: 1e-4 M of impact parameter over 1000 M)
+                const double inv = 1.0 / (double)ray.u0;
+                const double v1 = (double)ray.u1 * inv, v2 = (double)ray.u2 * inv, v3 = (double)ray.u3 * inv;
+                ray.u1 = (T)v1; ray.u2 = (T)v2; ray.u3 = (T)v3; ray.u0 = T(1);
+                car.u1 = (T)(v1 - (double)ray.u1); car.u2 = (T)(v2 - (double)ray.u2); car.u3 = (T)(v3 - (double)ray.u3);
+              } else {
+                T w = fastmath<T>::rcp(ray.u0);
+                ray.u1 *= w; ray.u2 *= w; ray.u3 *= w; ray.u0 = T(1);
+              }
             } else {
               lam = lam_in;
             }
             nst = nst0 = nst_in;
-            car.clear();
             have = true;
           }
         }
@@ -263,10 +273,16 @@ __device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n,
   const int32_t nst_in = s.nsteps[mine];
   if (st_in == GRAY2_ACTIVE) {
     sl.idx = mine;
+    clear_half<C>(car);
     if (FORM == 1) {
+      // v = u / u^t in double, split into the float the right-hand side sees and the residual of the compensated
+      // sum (see integrate_kernel)
       sl.lam = (double)t;
-      float w = fastmath<float>::rcp(u0);
-      u1 *= w; u2 *= w; u3 *= w; u0 = 1.0f;
+      const double inv = 1.0 / (double)u0;
+      const double v1 = (double)u1 * inv, v2 = (double)u2 * inv, v3 = (double)u3 * inv;
+      u1 = (float)v1; u2 = (float)v2; u3 = (float)v3; u0 = 1.0f;
+      set_half<C>(car.u1, (float)(v1 - (double)u1)); set_half<C>(car.u2, (float)(v2 - (double)u2));
+      set_half<C>(car.u3, (float)(v3 - (double)u3));
     } else {
       sl.lam = lam_in;
     }
@@ -274,7 +290,6 @@ __device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n,
     set_half<C>(ray.z, z); set_half<C>(ray.u0, u0); set_half<C>(ray.u1, u1);
     set_half<C>(ray.u2, u2); set_half<C>(ray.u3, u3);
     sl.nst = sl.nst0 = nst_in;
-    clear_half<C>(car);
     sl.have = true;
     sl.cap = false;
   }
