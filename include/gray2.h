@@ -19,7 +19,8 @@
  * gray2_integrate_diagnostics (the convergence measurements of section 3), gray2_convert plus
  * gray2_state.coords (the Boyer-Lindquist system of the paper's Table 2, behind the same gray2_integrate),
  * gray2_init_null_shard (one image shared by several GPUs), gray2_state.order plus
- * gray2_order_longest_first (an optional schedule of the integrators).
+ * gray2_order_longest_first (an optional schedule of the integrators), gray2_init_explicit_noalloc (explicit
+ * initial data for programs that must not allocate GPU memory).
  *
  * Memory and ownership.  Every pointer inside gray2_state, and every output array, is a DEVICE pointer
  * owned by the caller (e.g. a torch tensor) and only borrowed while the enqueued work runs.  The
@@ -28,7 +29,8 @@
  * the device, so any number of integrations may be in flight), the 32 KiB histogram of
  * gray2_order_longest_first (per device, allocated at its first call) and the staging buffers
  * of gray2_init_explicit (per device; n x 64 bytes each, one per calling stream up to eight, grown on demand,
- * reused, released at process exit).  `host_xu8` is a HOST pointer.
+ * reused, released at process exit).  Not allocated but part of the library's device code, and so held by every
+ * GPU that loads it: the fixed 4 MiB staging array of gray2_init_explicit_noalloc.  `host_xu8` is a HOST pointer.
  * gray2_state and gray2_step_control themselves are HOST structs, read during the call.
  *
  * Threads.  Any number of host threads may call into the library at once (the scratch pools are locked, the
@@ -144,6 +146,49 @@ int gray2_init_explicit(gray2_state *s, double a, const double *host_xu8, uint64
 /* The call north_star names: gray2_init_explicit with kind = GRAY2_TIMELIKE. */
 int gray2_init_timelike(gray2_state *s, double a, const double *host_xu8, uint64_t n,
                         int32_t renormalise_ut, void *cuda_stream);
+
+/* gray2_init_explicit for programs that must not allocate GPU memory: same arguments, same kernel, same state
+ * bit for bit, but the call allocates and frees nothing, on its first use or ever.
+ *
+ * Who needs it.  gray2_init_explicit parks the host array in a device buffer that the library owns and replaces
+ * (cudaFree, then cudaMalloc) whenever a call brings more geodesics than the slot of its stream has held so far.
+ * Which call does that depends on n and on the stream, so one warm-up call does not get it out of the way.  That
+ * is no good for
+ *   - a program that has handed nearly all of the GPU's memory to an allocator of its own (torch's caching
+ *     allocator after a large reservation, a renderer's arena, a job held to a fixed budget beside other tenants):
+ *     a cudaMalloc from inside this library fails there with out-of-memory, or takes memory the program counted on;
+ *   - a frame or control loop (the paper's interactive mode integrates and draws every frame):
+ *     cudaMalloc and cudaFree make the whole device wait, so the one call that grows the buffer stalls every other
+ *     stream for that frame;
+ *   - a program whose memory is checked once at start-up and locked down afterwards.
+ *
+ * What it uses instead.  A fixed staging array of GRAY2_NOALLOC_MAX_GEODESICS x 64 bytes = 4 MiB that is part
+ * of the library's device code: every GPU on which the library's kernels are loaded holds those 4 MiB from then
+ * until the process exits, whether this call is ever made or not.  n > GRAY2_NOALLOC_MAX_GEODESICS is refused
+ * with GRAY2_EINVAL (the error text names the limit) and nothing is enqueued: feed a larger batch in pieces,
+ * each piece into its own part of the state (a gray2_state whose pointers are offset), one after the other on
+ * one stream.
+ *
+ * First call on a device.  It looks up where the array lives on the current device (cudaGetSymbolAddress, which
+ * makes the CUDA runtime load the library's device code there if it has not yet) and keeps the answer; later
+ * calls on that device only enqueue.  Make that first call on each device while the program starts up, before
+ * any stream capture begins.
+ *
+ * One array for everybody.  All calls on a device, from any stream or host thread, stage through the same
+ * array, and it keeps what the last call left in it.  Nothing in it has to start at zero: the call overwrites
+ * the first 64 n bytes and its kernel reads exactly those, so old contents are never seen.  But two calls whose
+ * GPU work can overlap -- different streams with nothing ordering them -- write and read the array at the same
+ * time and both come out wrong; the library does not detect this.  Calls on one stream are safe (stream order),
+ * and so are calls on different devices (each device has its own copy of the array).
+ *
+ * The host array.  The copy is enqueued on cuda_stream itself (there is no internal stream and no event on this
+ * path), so unlike gray2_init_explicit the call does not wait for it: host_xu8 must stay valid and unchanged
+ * until cuda_stream has got past this call (pageable memory is read before the call returns, pinned memory when
+ * the stream reaches the copy).  Everything else -- kind, renormalise_ut, the fields set in s, the errors -- is
+ * as for gray2_init_explicit. */
+#define GRAY2_NOALLOC_MAX_GEODESICS 65536
+int gray2_init_explicit_noalloc(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t kind,
+                                int32_t renormalise_ut, void *cuda_stream);
 
 /* Integrate the first n geodesics of s (see gray2_step_control).  Only ACTIVE geodesics are touched, so
  * the call is resumable and a second identical call is a no-op.  prec must equal s->prec.

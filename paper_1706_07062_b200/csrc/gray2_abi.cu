@@ -642,3 +642,77 @@ int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per
 }
 
 }  // extern "C"
+
+// ---- gray2_init_explicit_noalloc: explicit initial data without any allocation -----------------------
+// gray2_init_explicit parks the caller's host array in a device buffer that the library cudaMallocs and, when a
+// later call brings more geodesics, cudaFrees and cudaMallocs again.  Programs that have given the GPU's memory to
+// an allocator of their own, that run a frame loop which a device-wide synchronisation would stall, or that lock
+// allocation down after start-up cannot have that (the full account is beside the declaration in gray2.h).  For
+// them the same kernel, init_explicit_kernel, reads its staging data from the array below instead: it is part of
+// the library's device image, so it costs its 4 MiB on every GPU that loads the library, from the load until the
+// process exits, called or not, and nobody ever allocates or frees it.
+//
+// g_noalloc_stage as written here in HOST code is only the host-side handle of the array, not a device address;
+// handing it to a kernel or to cudaMemcpy as a pointer would make the GPU fault (or, where the GPU can reach host
+// memory, quietly read the wrong bytes).  The device address is asked for once per device with
+// cudaGetSymbolAddress, that device being current, and every later call uses the address kept here.
+static __device__ __align__(256) double g_noalloc_stage[(size_t)GRAY2_NOALLOC_MAX_GEODESICS * 8];
+
+namespace {
+
+double *g_noalloc_addr[kMaxDevices] = {};   // device address of g_noalloc_stage on each device, NULL = not asked yet
+std::mutex g_noalloc_lock;
+
+// Device address of the staging array on the current device `dev`.  The first call per device does the look-up
+// (the runtime loads the library's device code on that device first if it has not yet); no memory is allocated.
+int noalloc_stage_of(int dev, double **out) {
+  std::lock_guard<std::mutex> guard(g_noalloc_lock);
+  if (!g_noalloc_addr[dev]) {
+    void *addr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&addr, g_noalloc_stage);
+    if (e != cudaSuccess || !addr)
+      return fail(GRAY2_ECUDA, "gray2_init_explicit_noalloc: cudaGetSymbolAddress of the staging array on device %d: %s",
+                  dev, cudaGetErrorString(e));
+    g_noalloc_addr[dev] = static_cast<double *>(addr);
+  }
+  *out = g_noalloc_addr[dev];
+  return GRAY2_OK;
+}
+
+}  // namespace
+
+extern "C" int gray2_init_explicit_noalloc(gray2_state *s, double a, const double *host_xu8, uint64_t n, int32_t kind,
+                                           int32_t renorm, void *cuda_stream) {
+  const char *who = "gray2_init_explicit_noalloc";
+  if (s) s->coords = GRAY2_KS;
+  int rc = check_state(s, who);
+  if (rc) return rc;
+  if (!host_xu8 || n == 0) return fail(GRAY2_EINVAL, "%s: host_xu8 is NULL or n == 0", who);
+  if (n > (uint64_t)GRAY2_NOALLOC_MAX_GEODESICS)
+    return fail(GRAY2_EINVAL, "%s: n = %llu is more than the %d geodesics (GRAY2_NOALLOC_MAX_GEODESICS) the fixed staging "
+                "array holds; split the batch, or use gray2_init_explicit if the program may allocate",
+                who, (unsigned long long)n, (int)GRAY2_NOALLOC_MAX_GEODESICS);
+  if (n > s->n) return fail(GRAY2_ESTATE, "%s: n (%llu) exceeds s->n (%llu)", who, (unsigned long long)n, (unsigned long long)s->n);
+  if (!(fabs(a) <= 1.0)) return fail(GRAY2_EINVAL, "%s: |a| must be <= 1 (got %g)", who, a);
+  if (kind != GRAY2_NULL && kind != GRAY2_TIMELIKE) return fail(GRAY2_EINVAL, "%s: kind must be GRAY2_NULL or GRAY2_TIMELIKE", who);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return fail(GRAY2_ECUDA, "device ordinal %d out of range", dev);
+  double *stage = nullptr;
+  rc = noalloc_stage_of(dev, &stage);
+  if (rc) return rc;
+  // Copy and kernel both go on the caller's stream: no internal stream and no events exist on this path.  The copy
+  // overwrites the first 64 n bytes of the array and the kernel reads exactly those, so whatever an earlier call
+  // left behind is never seen and nothing has to be cleared first.
+  const double mu2 = kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
+  CUDA_TRY(cudaMemcpyAsync(stage, host_xu8, (size_t)n * 8 * sizeof(double), cudaMemcpyHostToDevice, st));
+  unsigned grid = (unsigned)((n + 255) / 256);
+  if (s->prec == GRAY2_F64)
+    gray2::init_explicit_kernel<double><<<grid, 256, 0, st>>>(view_of<double>(s), stage, n, a, renorm, mu2);
+  else
+    gray2::init_explicit_kernel<float><<<grid, 256, 0, st>>>(view_of<float>(s), stage, n, a, renorm, mu2);
+  CUDA_TRY(cudaGetLastError());
+  s->a_eff = a; s->kind = kind; s->reversed = 0; s->coords = GRAY2_KS;
+  return GRAY2_OK;
+}

@@ -68,6 +68,8 @@ def load_library():
     lib.gray2_init_timelike.argtypes = [p, d, p, u64, i32, p]
     lib.gray2_init_explicit.argtypes = [p, d, p, u64, i32, i32, p]
     lib.gray2_init_explicit.restype = C.c_int
+    lib.gray2_init_explicit_noalloc.argtypes = [p, d, p, u64, i32, i32, p]
+    lib.gray2_init_explicit_noalloc.restype = C.c_int
     lib.gray2_init_null_shard.argtypes = [p, d, d, d, d, d, i32, i32, u64, i32, i32, p]
     lib.gray2_shard_count.argtypes = [u64, u64, i32, i32]
     lib.gray2_shard_count.restype = u64
@@ -198,6 +200,29 @@ def init_explicit(a, xu8, kind=NULL, prec=F64, renormalise_ut=False, stream=None
     _check(load_library().gray2_init_explicit(C.byref(cs), a, xu8.ctypes.data_as(C.c_void_p), n, int(kind),
                                               int(renormalise_ut), _stream_ptr(stream)))
     st._back(cs)
+    return st
+
+
+NOALLOC_MAX_GEODESICS = 65536      # GRAY2_NOALLOC_MAX_GEODESICS of include/gray2.h
+
+
+def init_explicit_noalloc(a, xu8, kind=NULL, prec=F64, renormalise_ut=False, stream=None,
+                          out: State | None = None) -> State:
+    """gray2_init_explicit_noalloc: init_explicit for programs that must not allocate GPU memory inside the library
+    (all of it promised to another allocator, a frame loop that a device-wide wait would stall, allocation locked
+    after start-up; see include/gray2.h).  The library stages through a fixed 4 MiB array instead of a buffer it
+    would cudaMalloc, so at most NOALLOC_MAX_GEODESICS geodesics per call (more raises Gray2Error, EINVAL), and calls
+    whose GPU work can overlap (different streams) race on that array.  Pass `out` to keep the state itself out of
+    torch's allocator as well.  The host array is kept alive on the returned State (``_host``) because the copy is
+    only enqueued: do not modify it before the stream has been synchronised."""
+    xu8 = _host_xu8(xu8)
+    n = xu8.shape[0]
+    st = out if out is not None else State.empty(n, prec)
+    cs = st._c()
+    _check(load_library().gray2_init_explicit_noalloc(C.byref(cs), a, xu8.ctypes.data_as(C.c_void_p), n, int(kind),
+                                                      int(renormalise_ut), _stream_ptr(stream)))
+    st._back(cs)
+    st._host = xu8
     return st
 
 

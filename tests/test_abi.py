@@ -228,3 +228,24 @@ def test_bench_line_blocks_are_assembled_from_the_measurements():
         if dtype == "f32":
             assert abs(r["frac_without_compensation_flops"] - r["frac"] * 530 / 554) < 1e-12
     assert bench.load_counters("cfg9", "f64", "affine") is None
+
+
+def test_noalloc_entry_states_its_limit_and_refuses_more_without_gpu_work(lib):
+    """gray2_init_explicit_noalloc stages through a fixed array (include/gray2.h): the limit is in the header, the
+    binding repeats it, and a larger batch is refused before any CUDA call with an error that names it."""
+    from paper_1706_07062_b200 import gray2
+    text = open(os.path.join(ROOT, "include", "gray2.h")).read()
+    limit = int(re.search(r"#define\s+GRAY2_NOALLOC_MAX_GEODESICS\s+(\d+)", text).group(1))
+    assert limit == gray2.NOALLOC_MAX_GEODESICS and limit * 64 == 4 << 20
+    s = gray2._CState()
+    s.n, s.prec = 1 << 20, 0
+    for m in range(8):
+        s.q[m] = 0x1000
+    s.lam = s.status = s.nsteps = 0x1000
+    fake, null = C.c_void_p(0x1000), C.c_void_p(0)
+    assert lib.gray2_init_explicit_noalloc(C.byref(s), 0.5, fake, limit + 1, 0, 0, null) == gray2.EINVAL
+    assert b"GRAY2_NOALLOC_MAX_GEODESICS" in lib.gray2_last_error() and str(limit).encode() in lib.gray2_last_error()
+    assert lib.gray2_init_explicit_noalloc(C.byref(s), 0.5, null, 16, 0, 0, null) == gray2.EINVAL     # no host array
+    assert lib.gray2_init_explicit_noalloc(C.byref(s), 0.5, fake, 16, 7, 0, null) == gray2.EINVAL     # unknown kind
+    s.n = 8
+    assert lib.gray2_init_explicit_noalloc(C.byref(s), 0.5, fake, 16, 0, 0, null) == gray2.ESTATE     # n > s->n
