@@ -88,7 +88,13 @@ typedef struct {
                         /* 8(a) a6, 8(b): "optional order array").  It changes the schedule only -- no       */
                         /* output bit depends on it -- and is used only by calls that cover all n geodesics.  */
                         /* Longest first shortens the tail of a launch (gray2_order_longest_first).           */
+                        /* A wrong array is data, not an error: an entry outside 0..n-1 is passed over; a       */
+                        /* geodesic listed twice is integrated by two lanes that store the same bits (its steps  */
+                        /* are counted twice in gray2_stats.steps); a geodesic listed nowhere is not touched      */
+                        /* and stays ACTIVE (gray2_stats.n_active tells).                                         */
 } gray2_state;
+/* Fill a gray2_state from zero (memset or = {0}): fields added by later versions of this header (`order` so far)
+ * mean "not used" when zero, and the library reads every field. */
 
 /* Step and stopping rule (DESIGN R4-R6).  For every geodesic with status ACTIVE, repeat:
  *   r = Kerr-Schild radius of the current position (eq. 5);
@@ -274,7 +280,8 @@ int gray2_invariants(const gray2_state *s, uint64_t n, double *E, double *Lz, do
  * every lane, and it is shortest when the short rays come last.  steps_hint, order: DEVICE arrays of n int32. */
 int gray2_order_longest_first(const int32_t *steps_hint, uint64_t n, int32_t *order, void *cuda_stream);
 
-/* Optional tuning of gray2_integrate's launch (0 = library default).  Results never depend on it. */
+/* Optional tuning of gray2_integrate's launch (0 = library default).  Results never depend on it.  Calls that
+ * follow a schedule (gray2_state.order) always run in the default shape: the ordered kernels exist for it only. */
 int gray2_set_launch(int32_t prec, int32_t threads_per_block, int32_t blocks_per_sm);
 
 /* Exact floating-point operation counts of one RK4 step of one geodesic in this library's code path

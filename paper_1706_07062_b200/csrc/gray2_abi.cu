@@ -48,7 +48,8 @@ struct Scratch {
   bool ready = false;
 };
 Scratch g_scratch[kMaxDevices];
-std::mutex g_scratch_lock;
+std::mutex g_scratch_lock;   // queue, done, next, num_sms, ready
+std::mutex g_order_lock;     // order_bins, order_done (gray2_order_longest_first only)
 
 struct QueueSlot {
   unsigned long long *queue, *steps;
@@ -84,10 +85,13 @@ int acquire_slot(cudaStream_t st, QueueSlot *out) {
 
 // ---- staging buffers of gray2_init_explicit: per device, one slot per calling stream -----------------
 constexpr int kStages = 8;
-struct Stage { cudaStream_t key; bool made; double *buf; size_t bytes; cudaEvent_t copied, consumed; };
+struct Stage {
+  cudaStream_t key; bool made; double *buf; size_t bytes; cudaEvent_t copied, consumed;
+  std::mutex mu;       // buf, bytes and the order of the work enqueued through this slot; key and made: g_stage_lock
+};
 struct StagePool { Stage slot[kStages] = {}; cudaStream_t copy_stream = nullptr; unsigned next = 0; };
 StagePool g_stages[kMaxDevices];
-std::mutex g_stage_lock;
+std::mutex g_stage_lock;     // which stream owns which slot, and the copy stream; never held across a wait
 
 // ---- launch configuration of the integrator (gray2_set_launch) ------------------------------------
 // (threads << 16) | blocks_per_sm in ONE atomic word per precision, 0 = default, so that an integration that
@@ -390,30 +394,43 @@ int gray2_init_explicit(gray2_state *s, double a, const double *host_xu8, uint64
   const size_t bytes = (size_t)n * 8 * sizeof(double);
   const double mu2 = kind == GRAY2_TIMELIKE ? 1.0 : 0.0;
   cudaEvent_t copied;
+  Stage *sl = nullptr;
+  cudaStream_t copy_stream = nullptr;
   {
+    // the pool-wide lock only while the slot is picked: growing a buffer (cudaFree, cudaMalloc, a wait for the kernel
+    // that last read it) and enqueueing happen under the slot's own lock, so that one thread's larger batch does not
+    // hold up the host-to-device copies of every other thread on every device
     std::lock_guard<std::mutex> guard(g_stage_lock);
     StagePool &pool = g_stages[dev];
     if (!pool.copy_stream) CUDA_TRY(cudaStreamCreateWithFlags(&pool.copy_stream, cudaStreamNonBlocking));
-    Stage *sl = nullptr;
+    copy_stream = pool.copy_stream;
     for (int i = 0; i < kStages && !sl; ++i)
       if (pool.slot[i].made && pool.slot[i].key == st) sl = &pool.slot[i];
     if (!sl) {
-      sl = &pool.slot[pool.next++ % kStages];
-      if (!sl->made) {
-        CUDA_TRY(cudaEventCreateWithFlags(&sl->copied, cudaEventDisableTiming));
-        CUDA_TRY(cudaEventCreateWithFlags(&sl->consumed, cudaEventDisableTiming));
-        sl->made = true;
+      Stage *cand = &pool.slot[pool.next % kStages];
+      if (!cand->made) {
+        cudaEvent_t e1 = nullptr, e2 = nullptr;
+        CUDA_TRY(cudaEventCreateWithFlags(&e1, cudaEventDisableTiming));
+        cudaError_t e = cudaEventCreateWithFlags(&e2, cudaEventDisableTiming);
+        if (e != cudaSuccess) { cudaEventDestroy(e1); return fail(GRAY2_ECUDA, "%s: cudaEventCreate: %s", who, cudaGetErrorString(e)); }
+        cand->copied = e1; cand->consumed = e2;
+        cand->made = true;
       }
-      sl->key = st;
+      pool.next++;
+      cand->key = st;
+      sl = cand;
     }
+  }
+  {
+    std::lock_guard<std::mutex> guard(sl->mu);
     if (bytes > sl->bytes) {
       if (sl->buf) { CUDA_TRY(cudaEventSynchronize(sl->consumed)); cudaFree(sl->buf); sl->buf = nullptr; sl->bytes = 0; }
       CUDA_TRY(cudaMalloc(&sl->buf, bytes));
       sl->bytes = bytes;
     }
-    CUDA_TRY(cudaStreamWaitEvent(pool.copy_stream, sl->consumed, 0));      // the kernel that last read this slot
-    CUDA_TRY(cudaMemcpyAsync(sl->buf, host_xu8, bytes, cudaMemcpyHostToDevice, pool.copy_stream));
-    CUDA_TRY(cudaEventRecord(sl->copied, pool.copy_stream));
+    CUDA_TRY(cudaStreamWaitEvent(copy_stream, sl->consumed, 0));      // the kernel that last read this slot
+    CUDA_TRY(cudaMemcpyAsync(sl->buf, host_xu8, bytes, cudaMemcpyHostToDevice, copy_stream));
+    CUDA_TRY(cudaEventRecord(sl->copied, copy_stream));
     CUDA_TRY(cudaStreamWaitEvent(st, sl->copied, 0));
     unsigned grid = (unsigned)((n + 255) / 256);
     if (s->prec == GRAY2_F64)
@@ -609,11 +626,22 @@ int gray2_order_longest_first(const int32_t *steps_hint, uint64_t n, int32_t *or
   CUDA_TRY(cudaGetDevice(&dev));
   if (dev < 0 || dev >= kMaxDevices) return fail(GRAY2_ECUDA, "device ordinal %d out of range", dev);
   constexpr int bins = gray2::kOrderBins;
-  std::lock_guard<std::mutex> guard(g_scratch_lock);        // one histogram per device: calls are serialised
+  // One histogram per device: calls are serialised, under a lock of their own (the first call allocates, and
+  // acquire_slot -- every integration of the process -- must not queue behind that).
+  std::lock_guard<std::mutex> guard(g_order_lock);
   Scratch &sc = g_scratch[dev];
   if (!sc.order_bins) {
-    CUDA_TRY(cudaMalloc(&sc.order_bins, (2 * bins + 1) * sizeof(unsigned)));
-    CUDA_TRY(cudaEventCreateWithFlags(&sc.order_done, cudaEventDisableTiming));
+    // the event first, and both published together: a failure leaves nothing half made for the next call
+    cudaEvent_t ev = nullptr;
+    unsigned *mem = nullptr;
+    CUDA_TRY(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    cudaError_t e = cudaMalloc(&mem, (2 * bins + 1) * sizeof(unsigned));
+    if (e != cudaSuccess) {
+      cudaEventDestroy(ev);
+      return fail(GRAY2_ECUDA, "gray2_order_longest_first: cudaMalloc of the histogram: %s", cudaGetErrorString(e));
+    }
+    sc.order_done = ev;
+    sc.order_bins = mem;
   }
   int sms = 0;
   CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));

@@ -141,8 +141,10 @@ integrate_kernel(StateView<T> s, uint64_t n, StepParams<T> p, unsigned long long
       if (base + cnt >= n) drained = true;
       if (!have) {
         uint64_t mine = base + __popc(idle & lt_mask);      // position in the queue
+        // ... and the geodesic the schedule puts there; an entry outside 0..n-1 (a negative one included: it
+        // converts to a huge index) names no geodesic and is passed over like the end of the queue
+        if constexpr (ORDERED) { if (mine < n) mine = (uint64_t)s.order[mine]; }
         if (mine < n) {
-          if constexpr (ORDERED) mine = (uint64_t)s.order[mine];   // ... and the geodesic the schedule puts there
           // the status and the state are fetched together (one round trip to memory instead of two); an entry
           // that turns out not to be ACTIVE is dropped and its slot of the lane refilled at the next pass
           const int32_t st_in = s.status[mine];
@@ -263,7 +265,10 @@ template <int C, int FORM, bool ORDERED>
 __device__ __forceinline__ void load_slot(const StateView<float> &s, uint64_t n, uint64_t mine, Ray<f32x2> &ray,
                                           Carry<f32x2> &car, PairSlot &sl) {
   if (mine >= n) return;
-  if constexpr (ORDERED) mine = (uint64_t)s.order[mine];
+  if constexpr (ORDERED) {
+    mine = (uint64_t)s.order[mine];
+    if (mine >= n) return;       // an entry outside 0..n-1 names no geodesic
+  }
   // the status and the state are fetched together (one round trip to memory instead of two)
   const int32_t st_in = s.status[mine];
   float t = s.q[0][mine], x = s.q[1][mine], y = s.q[2][mine], z = s.q[3][mine];

@@ -148,6 +148,7 @@ class State:
         s.coords = self.coords
         if self.order is not None:
             assert self.order.is_cuda and self.order.dtype == torch.int32 and self.order.numel() == self.n
+            assert self.order.is_contiguous() and self.order.device == self.q.device
             s.order = self.order.data_ptr()
         return s
 

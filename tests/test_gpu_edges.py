@@ -223,6 +223,42 @@ def test_set_launch_may_race_with_integrations():
     assert not errors, errors
 
 
+def test_init_explicit_from_four_threads_with_growing_batches():
+    """Any number of host threads (include/gray2.h "Threads"): four threads, a stream each, feed batches that keep
+    outgrowing their staging buffers, so that one thread's cudaFree + cudaMalloc runs while the others copy.  Every
+    state must hold exactly the rows its own thread passed in."""
+    import threading
+    errors = []
+
+    def worker(k):
+        try:
+            torch.cuda.set_device(0)
+            stream = torch.cuda.Stream()
+            rng = np.random.default_rng(100 + k)
+            for rnd, n in enumerate((257, 4099, 1000, 20011, 65537, 3, 131101)):
+                xu8 = rng.uniform(-40.0, 40.0, (n, 8))
+                prec = gray2.F64 if (rnd + k) % 2 == 0 else gray2.F32
+                with torch.cuda.stream(stream):
+                    g = gray2.init_explicit(0.3, xu8, gray2.NULL, prec=prec, stream=stream)
+                xu8_sent = xu8.copy()
+                xu8[:] = 0.0                  # the host array may be reused as soon as the call returns
+                stream.synchronize()
+                want = torch.tensor(xu8_sent.T, device="cuda").to(g.q.dtype)
+                if not torch.equal(g.q, want):
+                    errors.append((k, n, "state differs"))
+                if not bool((g.status == gray2.ACTIVE).all()) or not bool((g.nsteps == 0).all()):
+                    errors.append((k, n, "status / nsteps"))
+        except Exception as exc:              # noqa: BLE001 - reported by the main thread
+            errors.append((k, repr(exc)))
+
+    threads = [threading.Thread(target=worker, args=(k,)) for k in range(4)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
 def test_schedule_changes_no_output_bit():
     """gray2_state.order (optional order array): the longest-first order from a previous
     trace is a permutation sorted by decreasing step count, and integrating with it -- in both precisions, in
@@ -260,6 +296,39 @@ def test_schedule_changes_no_output_bit():
     hint = torch.tensor([5, 0, -3, 2_000_000_000, 17, 17, 1_000_000], dtype=torch.int32, device="cuda")
     o = gray2.order_longest_first(hint).cpu().numpy()
     assert sorted(o.tolist()) == list(range(7)) and o[0] == 3 and o[1] == 6
+
+
+def test_a_wrong_schedule_is_data_not_a_fault():
+    """gray2_state.order that is not a permutation (include/gray2.h): entries outside 0..n-1 are passed over, a geodesic
+    listed twice comes out with the bits of the unordered run, one listed nowhere is not touched and stays ACTIVE.
+    Both precisions (the one-per-thread and the packed ordered kernels)."""
+    cfg = inputs.CFG3_NULL.scaled(96, 64)
+    gsc, _ = image_sc(cfg)
+    n = cfg.n
+    rng = np.random.default_rng(8)
+    bad = rng.permutation(n).astype(np.int64)
+    left_out = bad[:500].copy()                       # these 500 positions get other contents:
+    bad[:100] = n + rng.integers(0, 1 << 20, 100)     #   beyond the end,
+    bad[100:200] = -1 - rng.integers(0, 1 << 20, 100) #   negative,
+    bad[200:300] = 0x7fffffff                         #   the largest int32,
+    bad[300:500] = bad[500:700]                       #   and 200 geodesics listed twice
+    listed = np.zeros(n, dtype=bool)
+    listed[bad[(bad >= 0) & (bad < n)]] = True
+    assert not listed[left_out].any() and listed.sum() == n - 500
+    for prec in (gray2.F64, gray2.F32):
+        ref = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=prec)
+        g = ref.clone()
+        start = ref.clone()
+        gray2.integrate(ref, INF, gsc)
+        g.order = torch.tensor(bad, dtype=torch.int32, device="cuda")
+        stats = gray2.new_stats()
+        gray2.integrate(g, INF, gsc, stats=stats)
+        torch.cuda.synchronize()
+        m = torch.tensor(listed, device="cuda")
+        assert torch.equal(g.q[:, m], ref.q[:, m]) and torch.equal(g.nsteps[m], ref.nsteps[m])
+        assert torch.equal(g.status[m], ref.status[m]) and torch.equal(g.lam[m], ref.lam[m])
+        assert torch.equal(g.q[:, ~m], start.q[:, ~m]) and bool((g.status[~m] == gray2.ACTIVE).all())
+        assert bool((g.nsteps[~m] == 0).all()) and gray2.stats_dict(stats)["n_active"] == 500
 
 
 def test_fma_probes_of_the_bench_run_in_every_form():
