@@ -607,8 +607,9 @@ int gray2_rhs_bl(int32_t prec, double a, uint64_t n, const void *pos, const void
 int gray2_flops_per_step(int32_t prec) { return prec == GRAY2_F32 ? 554 : 530; }
 
 /* Coordinate-time form: 4 x (107 + 6) + RK4 combination of six variables 80 + step rule and t update 2 = 534;
- * FP32: six compensated sums, + 18. */
-int gray2_flops_per_step_coordtime(int32_t prec) { return prec == GRAY2_F32 ? 552 : 534; }
+ * FP32: three compensated velocity sums, + 9, and the three positions advanced as x + h v + (h^2/6)(b_1 + b_2 + b_3)
+ * with the product h v carried exactly (advance_exact, ks_geodesic.cuh): 23 instead of 13 each, + 30, and h^2/6, + 1. */
+int gray2_flops_per_step_coordtime(int32_t prec) { return prec == GRAY2_F32 ? 574 : 534; }
 
 /* Boyer-Lindquist form, source-level count of bl_geodesic.cuh (same conventions):
  *   sin^2 and sin cos of theta: reduction 8, series 17 + 16, products 2 -> 43 (double: 8 / 8 terms, period pi/2),

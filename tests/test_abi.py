@@ -128,7 +128,7 @@ def test_new_entries_reject_bad_arguments_without_gpu_work(lib):
     assert lib.gray2_init_null_shard(C.byref(s), *args, 8, 0, 2, null) == EINVAL      # shard has 16 rays, state 15
     assert lib.gray2_rhs_bl(0, 0.5, 0, null, null, null, null) == EINVAL
     assert lib.gray2_flops_per_step_bl(0) == 598 and lib.gray2_flops_per_step_bl(1) == 590
-    assert lib.gray2_flops_per_step_coordtime(0) == 534 and lib.gray2_flops_per_step_coordtime(1) == 552
+    assert lib.gray2_flops_per_step_coordtime(0) == 534 and lib.gray2_flops_per_step_coordtime(1) == 574
     fake = C.c_void_p(0x1000)
     s.n = 16
     assert lib.gray2_init_explicit(C.byref(s), 0.5, fake, 16, 7, 0, null) == EINVAL   # unknown kind
