@@ -239,7 +239,9 @@ int gray2_convert(const gray2_state *src, gray2_state *dst, uint64_t n, int32_t 
  * vector of the same curve with another normalisation, so ratios such as L_z/E and Q/E^2 from
  * gray2_invariants keep their meaning.  s->lambda is not touched.  device_stats as for gray2_integrate.
  * FP32 states: the clock is q[0], a float, so t_end is rounded to float too: a geodesic that has reached the target
- * holds exactly float(t_end), and a second identical call is a no-op as in double.  Accuracy in FP32: as for
+ * holds exactly float(t_end), and a second identical call is a no-op as in double.  float(t_end) is the NEAREST
+ * float: the time reached may lie on either side of the t_end asked for, by up to half a float ulp of it (3e-5 M at
+ * t ~ 1000 M); pass a t_end that is a float already if the geodesics must not pass it.  Accuracy in FP32: as for
  * gray2_integrate, 1e-4 of max(|component|, r) on every geodesic that is not critical for FP32 (DESIGN R12); on 30
  * random images (spin, inclination, field of view, 100 M <= r_obs <= 2000 M, eta = 0.005 ... 0.02) the largest error
  * of such a geodesic is 1.4e-5, the median 3e-7 (tests/test_gpu_sweep.py).  The positions are advanced as

@@ -7,7 +7,7 @@ import torch
 
 import image_helpers as ih
 import oracle
-from gpu_helpers import (INF, TOL_STATE_F64, TWINS_ORBIT, accumulated_rounding_f64, assert_fp32_parity, image_sc, image_sc_kw, make_straddle_check, run_gpu_image,
+from gpu_helpers import (INF, TOL_STATE_F32, TOL_STATE_F64, TWINS_ORBIT, accumulated_rounding_f64, assert_fp32_parity, image_sc, image_sc_kw, make_straddle_check, run_gpu_image,
                          sc_pair, state_rel_error, take, to_oracle_state, twin_sensitivity)
 from paper_1706_07062_b200 import gray2, inputs
 
@@ -123,7 +123,7 @@ def test_fp32_packed_and_scalar_kernels_agree_bit_for_bit():
     cfg = inputs.CFG3_NULL.scaled(150, 91)          # odd ray count: the last thread has an empty second slot
     ref = None
     try:
-        for shape in [(0, 0), (128, 3), (128, 4), (128, 8), (128, 6)]:
+        for shape in [(0, 0), (256, 2), (256, 1), (128, 3), (128, 4), (128, 8), (128, 6)]:
             gray2.set_launch(gray2.F32, *shape)
             _, g, stats = run_gpu_image(cfg, prec=gray2.F32)
             cur = (g.q.clone(), g.nsteps.clone(), g.status.clone(), g.lam.clone(), stats)
@@ -420,6 +420,78 @@ def test_full_size_image_sampled_parity(cfg, nsample):
     assert abs(gstats["n_captured"] / cfg.n - area / (2 * cfg.fov) ** 2) < 2e-3
 
 
+@pytest.mark.parametrize("form", ["affine", "coordtime"])
+def test_fp32_trace_split_into_calls_stays_within_rounding(form):
+    """An FP32 state is plain float at every call boundary (include/gray2.h): the residuals of the compensated sums are
+    dropped when a geodesic is stored, so a trace made in several calls differs from the same trace made in one -- by
+    one float rounding of the state per call, which the geodesic then carries like a rounding of its input.  Bounded
+    here: eight segments against one call, every ray that is not critical for FP32 (the criterion of the parity tests)
+    ends with the same status, on the same line of flight: the impact vector x x v_hat, which does not depend on where
+    along the ray the two traces stop, agrees to a few float ulp of r."""
+    cfg = inputs.CFG3_NULL.scaled(80, 64)
+    gsc, _ = image_sc(cfg)
+    kw = image_sc_kw(cfg)
+    run = gray2.integrate_coordtime if form == "coordtime" else gray2.integrate
+    one = gray2.init_null(cfg.a, cfg.r_obs, cfg.inclination, cfg.fov, cfg.fov, cfg.nx, cfg.ny, prec=gray2.F32)
+    o0 = to_oracle_state(one)
+    many = one.clone()
+    run(one, INF, gsc)
+    for end in (150.0, 400.0, 700.0, 900.0, 980.0, 1010.0, 1300.0, INF):      # lambda or t: about the same far out
+        run(many, end, gsc)
+    torch.cuda.synchronize()
+    a, b = to_oracle_state(one), to_oracle_state(many)
+    sens = twin_sensitivity(o0, kw)
+    noncrit = sens <= TOL_STATE_F32
+    assert noncrit.mean() > 0.9 and np.array_equal(a.status[noncrit], b.status[noncrit])
+    # a call that ends at lambda_end clips its last step, so the split trace has up to seven steps more
+    assert (np.abs(a.nsteps - b.nsteps)[noncrit] <= 8).all() and (b.nsteps >= a.nsteps)[noncrit].all()
+    near = noncrit & (np.abs(a.nsteps - b.nsteps) <= 8)
+    r_a = np.array([oracle.ks_r(a.a_eff, *a.q[1:4, k]) for k in range(a.n)])
+    # the two traces stop a few (clipped) steps apart: compare what does not depend on where along the ray they stop
+    va, vb = a.q[5:8] / np.linalg.norm(a.q[5:8], axis=0), b.q[5:8] / np.linalg.norm(b.q[5:8], axis=0)
+    dv = np.linalg.norm(va - vb, axis=0)          # up to 8 steps further out the ray has bent by up to ~2 b dr / r^2 ~ 1e-5
+    bvec_a = np.cross(a.q[1:4].T, va.T)           # impact vector x x v_hat: constant far out
+    bvec_b = np.cross(b.q[1:4].T, vb.T)
+    db = np.linalg.norm(bvec_a - bvec_b, axis=1) / r_a
+    esc = near & (a.status == gray2.ESCAPED)
+    print("[fp32 split calls] %s: direction differs by median %.2e max %.2e, impact vector / r by median %.2e max %.2e (%d escaped rays)"
+          % (form, np.median(dv[esc]), dv[esc].max(), np.median(db[esc]), db[esc].max(), esc.sum()))
+    # measured: impact vector / r median 3e-8, max 1.4e-7 (half a float ulp is 3e-8)
+    assert dv[esc].max() < TOL_STATE_F32 and db[esc].max() < 2e-6 and np.median(db[esc]) < 2e-7
+
+
+def test_full_size_headline_image_fp32_sampled_parity():
+    """cfg3 at 1024 x 1024 in FP32 -- the workload and the kernel (packed 256 x 2, the default at this size) of the
+    bench line's fp32 block -- against 1,536 sampled oracle rays fed the float initial state: north_star's FP32 clause
+    on every non-critical sampled ray.  Also printed: how many of the rays the criterion excludes were within 1e-4
+    anyway, so that its slack stays visible."""
+    cfg = inputs.CFG3_NULL
+    g0, g, gstats = run_gpu_image(cfg, prec=gray2.F32)
+    assert gstats["n_active"] == 0 and gstats["n_invalid"] == 0 and gstats["n_maxsteps"] <= 2
+    assert gstats["steps"] == int(g.nsteps.sum(dtype=torch.int64).item())
+    rng = np.random.default_rng(1706)
+    idx = np.sort(rng.choice(cfg.n, 1536, replace=False))
+    o0 = take(to_oracle_state(g0), idx)              # the same inputs: the float initial state, widened
+    o = o0.copy()
+    kw = image_sc_kw(cfg)
+    oracle.integrate(o, INF, oracle.step_control(**kw))
+    gst = take(to_oracle_state(g), idx)
+    sens = twin_sensitivity(o0, kw)
+    err = state_rel_error(gst.q, o.q, o.a_eff)
+    noncrit, same = assert_fp32_parity(cfg.name + " full size, sampled", gst, o, sens, err, make_straddle_check(o0, gst, o, kw))
+    agree = (gst.status == o.status) & (gst.nsteps == o.nsteps)
+    fine_anyway = int(((~noncrit) & agree & (err < TOL_STATE_F32)).sum())
+    print("[fp32 parity] %s: of the %d sampled rays excluded as critical, %d were within %.0e anyway; beyond it on all rays: %d"
+          % (cfg.name, int((~noncrit).sum()), fine_anyway, TOL_STATE_F32, int((~(agree & (err < TOL_STATE_F32))).sum())))
+    xi, eta, _, _ = ih.ray_constants(o0)
+    mask = ih.potential_mask(o0.a_eff, xi, eta, 900.0)
+    assert np.array_equal((gst.status == gray2.CAPTURED)[noncrit], mask[noncrit])
+    ca, cb = __import__("closed_forms").bardeen_curve(cfg.a, cfg.inclination)
+    order = np.argsort(ca)
+    area = 2.0 * np.trapezoid(cb[order], ca[order])
+    assert abs(gstats["n_captured"] / cfg.n - area / (2 * cfg.fov) ** 2) < 2e-3
+
+
 def test_cfg4_ensemble_sample_parity_and_drift():
     xu8, meta = inputs.cfg4_ensemble(4096)
     gsc, osc = sc_pair(mode=0, h_fixed=0.5, max_steps=3000)
@@ -442,6 +514,9 @@ def test_cfg4_ensemble_sample_parity_and_drift():
     noncrit = sens <= TOL_STATE_F64
     print("[cfg4 sample] %d of 4096 orbits critical; max error on the others %.2e, on all %.2e" % ((~noncrit).sum(), err[noncrit].max(), err.max()))
     assert noncrit.mean() > 0.99 and err[noncrit].max() < TOL_STATE_F64, (noncrit.mean(), err[noncrit].max())
+    # and without any criterion: every orbit within 10 x the tolerance (measured 7.4e-10), the criterion excluding
+    # no more than a handful (measured 3 of 4096)
+    assert err.max() < 10 * TOL_STATE_F64 and (~noncrit).sum() <= 8, (err.max(), (~noncrit).sum())
     gi1 = [t.cpu().numpy() for t in gray2.invariants(g)]
     oi1 = oracle.invariants(o)
     from gpu_helpers import invariant_term_scales
@@ -491,6 +566,11 @@ def test_cfg4_full_size_sampled_parity():
     print("[cfg4 full size] critical or plunged: %d of the 512 evenly spaced, %d of the 256 deepest; max error on the others %.2e"
           % ((~noncrit[:512]).sum(), (~noncrit[512:]).sum(), err[noncrit].max()))
     assert noncrit[:512].mean() > 0.95 and err[noncrit].max() < TOL_STATE_F64, (noncrit[:512].mean(), err[noncrit].max())
+    # Unconditional ceilings beside the criterion, from the recorded run (evenly spaced: max 1.07e-9, 20 of 512 excluded;
+    # deepest periapses: max 4.3e-7 over the orbiting ones, 101 of 256 excluded): the criterion may not hide an orbit that
+    # is off by more than the phase growth of 1e5 steps explains, nor grow to exclude more than it does today.
+    assert err[:512][orbiting[:512]].max() < 1e-8 and err[512:][orbiting[512:]].max() < 5e-6
+    assert (~noncrit[:512]).sum() <= 26 and (~noncrit[512:]).sum() <= 115, ((~noncrit[:512]).sum(), (~noncrit[512:]).sum())
     gi1 = [t.cpu().numpy() for t in gray2.invariants(g)]
     oi1 = oracle.invariants(o)
     from gpu_helpers import invariant_term_scales

@@ -181,11 +181,19 @@ def test_kerr_images_reduced_resolution_full_parity(cfg):
     assert abs(gstats["steps"] - ostats["steps"]) <= 40 * (~outside).sum()
 
 
+@pytest.mark.parametrize("launch", [(0, 0), (256, 2)], ids=["default-launch", "packed-256x2"])
 @pytest.mark.parametrize("cfg", [inputs.CFG3_NULL.scaled(64), inputs.CFG1_NULL, inputs.CFG2_NULL.scaled(72, 56)],
                          ids=lambda c: c.name)
-def test_fp32_against_oracle(cfg):
-    """north_star's FP32 clause on EVERY non-critical ray, all eight components (DESIGN R12; gpu_helpers)."""
-    g0, g, gstats = run_gpu_image(cfg, prec=gray2.F32)
+def test_fp32_against_oracle(cfg, launch):
+    """north_star's FP32 clause on EVERY non-critical ray, all eight components (DESIGN R12; gpu_helpers).  Images this
+    small get the one-per-thread float kernel by default (gray2_abi.cu, small batches); the second launch forces the
+    packed two-per-thread kernel that full-size images -- and bench.py -- run.  (The coordinate-time and
+    Boyer-Lindquist forms have the packed kernel only, at every size.)"""
+    gray2.set_launch(gray2.F32, *launch)
+    try:
+        g0, g, gstats = run_gpu_image(cfg, prec=gray2.F32)
+    finally:
+        gray2.set_launch(gray2.F32, 0, 0)
     o0 = to_oracle_state(g0)                        # the same inputs: the float initial state, widened
     o = o0.copy()
     kw = image_sc_kw(cfg)
