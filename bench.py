@@ -69,6 +69,18 @@ def load_measured_peaks():
         return {}
 
 
+def csrc_digest() -> str:
+    """First 12 hex digits of the SHA-256 over the library's kernel sources and its header (sorted by name): the
+    stamp of profiles/kernel_counters.csv rows (column csrc_sha12), so that a row captured on other kernels shows."""
+    import hashlib
+    csrc = os.path.join(ROOT, "paper_1706_07062_b200", "csrc")
+    h = hashlib.sha256()
+    for path in sorted(os.path.join(csrc, f) for f in os.listdir(csrc)) + [os.path.join(ROOT, "include", "gray2.h")]:
+        with open(path, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
 def load_counters(workload: str, dtype: str, form: str):
     """Row of profiles/kernel_counters.csv for (workload, dtype, form), or None."""
     try:
@@ -322,7 +334,7 @@ def measure(job: Job, dtype: str) -> dict:
     # ---- device-resident: exactly K steps, L2 flushed before each, CUDA events on the launching stream
     job.barrier()
     t_window0 = time.perf_counter()
-    per_step, per_int, steps_total = [], [], 0
+    per_step, per_int, per_init, per_inv, steps_total = [], [], [], [], 0
     for _ in range(args.steps):
         job.flush.fill_(1)                                     # flush L2 between timed iterations (untimed)
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
@@ -330,6 +342,8 @@ def measure(job: Job, dtype: str) -> dict:
         ev[3].synchronize()
         per_step.append(ev[0].elapsed_time(ev[3]) * 1e-3)
         per_int.append(ev[1].elapsed_time(ev[2]) * 1e-3)
+        per_init.append(ev[0].elapsed_time(ev[1]) * 1e-3)
+        per_inv.append(ev[2].elapsed_time(ev[3]) * 1e-3)
         steps_total += int(stats[0].item())
     job.barrier()
     clocks = job.sampler.window(t_window0, time.perf_counter())
@@ -412,7 +426,8 @@ def measure(job: Job, dtype: str) -> dict:
         probe[name] = (32 if regs == 3 else 16) * iters * blocks * threads / (e0.elapsed_time(e1) * 1e-3) / 1e12
     if args.threads or args.blocks:
         gray2.set_launch(prec, 0, 0)
-    return dict(dtype=dtype, prec=prec, per_step=per_step, per_int=per_int, steps_total=steps_total, clocks=clocks,
+    return dict(dtype=dtype, prec=prec, per_step=per_step, per_int=per_int, per_init=per_init, per_inv=per_inv,
+                steps_total=steps_total, clocks=clocks,
                 t_e2e=t_e2e, e2e_steps=e2e_steps, h2d=h2d, d2h=d2h, n_chunks=n_chunks, n_streams=n_streams,
                 probe=probe, warmup=warmup)
 
@@ -505,6 +520,12 @@ def block_of(job: Job, m: dict, t_step, t_int, steps_all, t_e2e, e2e_all) -> dic
                 "api": "gray2_init_explicit(host 8-vectors, NULL) -> %sgray2_integrate -> gray2_invariants -> D2H of state, invariants, stats"
                        % ("gray2_convert -> " if job.bl else ""),
                 "chunks": m["n_chunks"], "streams": m["n_streams"]},
+        # SURVEY 8(d) "also report init time, invariants time": this rank's mean per step, CUDA events around
+        # gray2_init_null (+ gray2_convert for --form bl) and around gray2_invariants
+        "init_ms": 1e3 * statistics.mean(m["per_init"]) if m.get("per_init") else None,
+        "invariants_ms": 1e3 * statistics.mean(m["per_inv"]) if m.get("per_inv") else None,
+        # kernels of this library per step: init_null, integrate, count_status, invariants (+ ks_to_bl).  gray2_integrate
+        # also enqueues two memsets and one 8-byte device-to-device copy, which are not kernels of the library.
         "gpu_launches": (5 if job.bl else 4) * args.steps,
         "roofline": {"bound": "alu", "kernel": kernel,
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
@@ -512,13 +533,16 @@ def block_of(job: Job, m: dict, t_step, t_int, steps_all, t_e2e, e2e_all) -> dic
                      "executed_frac": (m["steps_total"] * exec_flops / sum(m["per_int"]) / 1e12 / peak) if exec_flops else None,
                      "executed_flops_per_rk4_step": exec_flops,
                      "executed_source": row.get("executed_source"),
+                     # the profiler-only figures were captured on the build whose kernel sources hash to the row's
+                     # csrc_sha12; False = the kernels have changed since, executed_frac and traffic describe an older build
+                     "counters_match_this_build": (row.get("csrc_sha12") == csrc_digest()) if row else None,
                      "traffic": traffic,
                      "traffic_unit": "bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum, profiles/kernel_counters.csv)",
                      "algorithmic_bytes": 2 * (80 if dtype == "f64" else 48) * job.n_local,
                      "flops_per_rk4_step": fps,
                      # FP32 only: the same fraction with the count of the uncompensated step (round 1's: 530 affine,
                      # 534 coordinate time, 566 Boyer-Lindquist), i.e. without the 3 additions per state variable
-                     "frac_without_compensation_flops": (achieved / peak) * (fps - (18 if job.coord else 24)) / fps
+                     "frac_without_compensation_flops": (achieved / peak) * (566 if job.bl else job.flops_per_step(job.gray2.F64)) / fps
                                                         if dtype == "f32" else None,
                      "kernel_ms": 1e3 * t_int / args.steps, "kernel_ms_best": 1e3 * best_int,
                      "kernel_share_of_step": t_int / t_step,

@@ -1,6 +1,6 @@
 """Run the five BASELINE.json configs on the GPU and print one JSON report (GPU-only statistics).
 
-    python -m paper_1706_07062_b200.report [--configs 1,2,3,4,5] [--cfg4-steps 100000] [--cfg4-n 1048576]
+    python report.py [--configs 1,2,3,4,5] [--cfg4-steps 100000] [--cfg4-n 1048576]
 
 What each config asks to be reported (BASELINE.json "configs"):
   cfg1  Schwarzschild 64x64 image + 16 time-like orbits: status counts, step counts, invariant drift
@@ -9,7 +9,7 @@ What each config asks to be reported (BASELINE.json "configs"):
         rays and on the capture mask
   cfg4  1,048,576 bound particles, fixed step 0.5, 100,000 steps: drift of E, L_z, Q and u.u
   cfg5  Kerr a=0.5 4096x4096 in FP32 and FP64: throughput under divergence in path length
-The oracle comparisons live in tests/ (this module never touches the oracle).
+The oracle comparisons live in tests/ (this script never touches the oracle).  It is harness, like bench.py: it sits beside it, outside the library package.
 """
 from __future__ import annotations
 
@@ -20,7 +20,11 @@ import time
 
 import torch
 
-from . import gray2, inputs
+import os
+import sys
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+from paper_1706_07062_b200 import gray2, inputs  # noqa: E402
 
 INF = float("inf")
 

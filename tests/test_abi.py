@@ -211,7 +211,8 @@ def test_bench_line_blocks_are_assembled_from_the_measurements():
     for dtype, prec in (("f64", F64), ("f32", F32)):
         m = dict(dtype=dtype, prec=prec, per_step=[0.030, 0.028], per_int=[0.0295, 0.0275], steps_total=2_200_000_000,
                  clocks={"sm_mhz": 1965.0, "reasons": []}, h2d=64, d2h=80, n_chunks=32, n_streams=8,
-                 probe={"imm": 36.0, "regs": 34.0, "fresh": 24.6, "packed": 48.7}, warmup=3)
+                 probe={"imm": 36.0, "regs": 34.0, "fresh": 24.6, "packed": 48.7}, warmup=3,
+                 per_init=[17e-6, 19e-6], per_inv=[16e-6, 16e-6])
         b = bench.block_of(job, m, t_step=0.058, t_int=0.057, steps_all=2.2e9, t_e2e=0.06, e2e_all=2.2e9)
         peak = 148 * (64 if dtype == "f64" else 128) * 2 * 1965e6 / 1e12
         assert abs(b["value"] - 2.2e9 / 0.058) < 1 and abs(b["ms_per_step"] - 29.0) < 1e-9
@@ -225,6 +226,8 @@ def test_bench_line_blocks_are_assembled_from_the_measurements():
         assert r["algorithmic_bytes"] == 2 * (80 if dtype == "f64" else 48) * (1 << 20)
         assert b["e2e"]["h2d_bytes_per_step"] == 64 and abs(b["e2e"]["value"] - 2.2e9 / 0.06) < 1
         assert b["gpu_launches"] == 8
+        assert abs(b["init_ms"] - 0.018) < 1e-12 and abs(b["invariants_ms"] - 0.016) < 1e-12
+        assert r["counters_match_this_build"] == (row.get("csrc_sha12") == bench.csrc_digest())
         if dtype == "f32":
             assert abs(r["frac_without_compensation_flops"] - r["frac"] * 530 / 554) < 1e-12
     assert bench.load_counters("cfg9", "f64", "affine") is None
